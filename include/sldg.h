@@ -1,0 +1,134 @@
+/*
+ * sldg.h -- C-ABI boundary of the B200-native SLDG Vlasov-Poisson hot path
+ * (arXiv:1907.08316, "Semi-Lagrangian Vlasov simulation on GPUs").
+ *
+ * Citations: "P:n" = line n of the paper text; "D:Rx / D:Ox" = the
+ * readings and definitions listed in DESIGN.md (taken from SURVEY.md section 8(c)).
+ *
+ * What the library computes (section 1, section 2, section 3):
+ *   - the semi-Lagrangian discontinuous-Galerkin translation of f along one
+ *     phase-space direction: in every cell the o Gauss-Legendre nodal values become
+ *         u_new[i][j] = sum_l A_jl u_old[i*][l] + sum_l B_jl u_old[i*+1][l]
+ *     with A(theta), B(theta) in R^{o x o} the L2 projection of the exactly shifted
+ *     piecewise polynomial, applied "for each slice of the high-dimensional
+ *     problem";
+ *   - rho(x) = -int f dv, the periodic Poisson problem -Lap phi = rho + 1,
+ *     E = -grad phi, the Strang step and the invariants mass, L2 norm and
+ *     electric energy.
+ *
+ * Layout of f at this boundary ("canonical"): dense array of N = prod_d N_d values,
+ * N_d = cells[d]*order, dimensions ordered x_1..x_dx, v_1..v_dv, linear index
+ * sum_d p_d * prod_{e<d} N_e (x_1 fastest), node index p_d = i_d*order + j_d (cell i_d,
+ * local Gauss-Legendre node j_d, nodes ascending).  All directions are periodic (D:R5).
+ *
+ * Memory: the two f buffers are CALLER-owned DEVICE memory (N*sizeof(T) bytes each,
+ * 16-byte aligned); the library ping-pongs between them and allocates only small
+ * tables (A/B, rho, E, partial sums, DFT matrices) of size O(X + sum N_d + splits*X).
+ * Streams: every call enqueues on the stream given to sldg_create and returns without
+ * synchronising, except where stated.
+ *
+ * Errors: every int-returning call returns SLDG_OK (0) or a negative sldg_status; the
+ * library never throws, exits or falls back to a CPU path.  sldg_last_error() gives a
+ * human-readable message for the last failure on that context (or the last failed
+ * sldg_create when ctx == NULL).
+ */
+#ifndef SLDG_H
+#define SLDG_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sldg_ctx sldg_ctx;            /* opaque; owned by the library            */
+
+typedef enum { SLDG_F64 = 0, SLDG_F32 = 1 } sldg_dtype;   /* storage/arithmetic type T of f */
+
+typedef enum {
+    SLDG_OK = 0,
+    SLDG_ERR_ARG = -1,          /* null pointer, dimension/order/count out of range      */
+    SLDG_ERR_UNSUPPORTED = -2,  /* (order, dtype, dims) combination not instantiated     */
+    SLDG_ERR_CUDA = -3,         /* a CUDA runtime call or kernel launch failed           */
+    SLDG_ERR_STATE = -4         /* call needs something not yet computed (E, rho, f)     */
+} sldg_status;
+
+#define SLDG_MAX_DIM 6
+#define SLDG_MAX_ORDER 4
+
+/* Create a solver context (template parameters (d_x, d_v, o) become run-time here).
+ *   dx, dv      1..3 each, dv >= dx (E has dx components and accelerates v_1..v_dx)
+ *   cells       [dx+dv] host ints, n_d >= 1
+ *   order       o in 1..SLDG_MAX_ORDER (number of Gauss-Legendre nodes per cell per dim)
+ *   lo, hi      [dx+dv] host doubles, hi > lo
+ *   f_buf0/1    device pointers, N*sizeof(T) bytes each, distinct, not freed by the library
+ *   cuda_stream a cudaStream_t (0 = legacy default stream)
+ * The current buffer is f_buf0 until a sweep flips it. */
+int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int order,
+                const double *lo, const double *hi, sldg_dtype dtype,
+                void *f_buf0, void *f_buf1, void *cuda_stream);
+
+/* Synchronises the stream, frees the library's tables.  The f buffers stay the caller's. */
+int sldg_destroy(sldg_ctx *ctx);
+
+const char *sldg_last_error(const sldg_ctx *ctx);
+
+size_t sldg_num_dofs(const sldg_ctx *ctx);          /* N                                   */
+size_t sldg_num_x(const sldg_ctx *ctx);             /* X = prod_{d<dx} N_d                 */
+
+/* Node coordinates c_d(p) = lo_d + (i + xi_j) h_d, p = i*o + j, host_out[N_dim].   */
+int sldg_node_coords(const sldg_ctx *ctx, int dim, double *host_out);
+
+/* Copy N values of type T into / out of the current buffer.  Host copies use
+ * cudaMemcpyAsync on the stream followed by a stream synchronise. */
+int sldg_set_initial(sldg_ctx *ctx, const void *f_src, int is_device);
+int sldg_get_f(sldg_ctx *ctx, void *dst, int is_device);
+void *sldg_current(sldg_ctx *ctx);                  /* device pointer holding f now        */
+
+/* Fill the current buffer with f[g] = U(seed, tag, g) in [0,1) rounded to T, g = canonical
+ * linear index: the counter-based generator of the config-4 microbenchmark (DESIGN.md
+ * "Input recipe"; splitmix64 finaliser, top 53 bits * 2^-53). */
+int sldg_fill_uniform(sldg_ctx *ctx, unsigned long long seed, unsigned tag);
+
+/* Row a-1 + a-2: raw translation sweep along dimension `dim` (0-based), the
+ * shift sigma_q of every line given in CELL WIDTHS (new(x) = old(x - sigma h), D:R3):
+ *   dim <  dx (x_a):  count = N_{v_a},  q = node index of v_a
+ *   dim >= dx (v_a):  count = X,        q = x-node index (x_1 fastest)
+ * shift_cells is a HOST array read before the call returns.  Flips the current buffer. */
+int sldg_translate(sldg_ctx *ctx, int dim, const double *shift_cells_host, size_t count);
+
+/* As sldg_translate but the shift table is already in DEVICE memory (fp64) and is read
+ * on the stream; nothing is copied from the host.  This is what the microbenchmark times. */
+int sldg_translate_dev(sldg_ctx *ctx, int dim, const double *shift_cells_device, size_t count);
+
+/* Physics sweep (D:O3, D:R4): dim < dx: sigma = c_{v_a}(q) dt / h_{x_a};
+ * dim >= dx: sigma = -E_a(x_q) dt / h_{v_a} with the stored E (SLDG_ERR_STATE if none). */
+int sldg_advect(sldg_ctx *ctx, int dim, double dt);
+
+/* rho[X] = -sum_v W_v f[v][x] (fp64 accumulation for both dtypes) into the
+ * context and, if rho_device_or_null != NULL, also to that device array. */
+int sldg_compute_rho(sldg_ctx *ctx, double *rho_device_or_null);
+
+/* E[dx][X] from the stored rho: -Lap phi = rho + 1 periodic, E = -grad phi at the x-nodes,
+ * spectral with the modes |m_a| <= floor((n_a - 1)/2) and the mean mode dropped (D:R6, D:R13). */
+int sldg_poisson_E(sldg_ctx *ctx, double *E_device_or_null);
+
+/* Overwrite the stored E ([dx][X] fp64, host or device): lets a caller drive sldg_advect in v. */
+int sldg_set_E(sldg_ctx *ctx, const double *E, int is_device);
+
+/* Strang step (D:O6 row a-5): x_1..x_dx with dt/2, rho, Poisson, v_1..v_dx with dt,
+ * x_1..x_dx with dt/2. */
+int sldg_step(sldg_ctx *ctx, double dt);
+
+/* mass = sum W f, l2 = sqrt(sum W f^2), electric_energy = 1/2 sum_x W_x |E|^2 from the
+ * current f (D:R12); recomputes rho and E; synchronises the stream.  Any of the three
+ * output pointers (host) may be NULL. */
+int sldg_diagnostics(sldg_ctx *ctx, double *mass, double *l2, double *electric_energy);
+
+/* Number of kernels this context has launched since sldg_create (bench "gpu_launches"). */
+unsigned long long sldg_launch_count(const sldg_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SLDG_H */

@@ -1,0 +1,123 @@
+// reduce.cuh -- rows a-3 and a-6: rho(x) = -sum_v W_v f[v][x] and the invariants mass,
+// L2 norm, electric energy (D:R12).  fp64 accumulators for both storage types and a
+// hierarchical, deterministic reduction thread -> split -> final pass.
+//
+// In the canonical layout the reduced index v is the SLOW one, so the bulk of the work is a
+// per-thread column sum over a range of v (coalesced, 128-bit loads along x); the ranges
+// ("splits") exist only to expose enough parallelism.  Full reductions to a scalar over the
+// X-sized results use warp shuffles + one shared-memory stage in a single block.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "sweep.cuh"   // Vec<T,VEC>
+
+namespace sldg {
+
+// part_rho[split][x] = sum_{v in split} W_v f[v][x];  part_s2 likewise with f^2 (if WITH_S2)
+template <typename T, int VEC, bool WITH_S2, int UB>
+__global__ void __launch_bounds__(256)
+vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
+                    const double *__restrict__ Wv, double *__restrict__ part_rho,
+                    double *__restrict__ part_s2) {
+    using Vt = Vec<T, VEC>;
+    const long xv = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long x = xv * VEC;
+    if (x >= X) return;
+    const long split = blockIdx.y;
+    const long v0 = split * vps;
+    long v1 = v0 + vps;
+    if (v1 > V) v1 = V;
+    double acc[VEC], acc2[VEC];
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) { acc[e] = 0.0; acc2[e] = 0.0; }
+    const T *p = f + v0 * X + x;
+    long v = v0;
+    for (; v + UB <= v1; v += UB) {
+        Vt u[UB];
+        double w[UB];
+#pragma unroll
+        for (int b = 0; b < UB; ++b) {
+            u[b] = *reinterpret_cast<const Vt *>(p + (long)b * X);
+            w[b] = Wv[v + b];
+        }
+#pragma unroll
+        for (int b = 0; b < UB; ++b)
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) {
+                double val = (double)u[b].v[e];
+                double wv = w[b] * val;
+                acc[e] += wv;
+                if (WITH_S2) acc2[e] = fma(wv, val, acc2[e]);
+            }
+        p += (long)UB * X;
+    }
+    for (; v < v1; ++v) {
+        Vt u = *reinterpret_cast<const Vt *>(p);
+        double w = Wv[v];
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) {
+            double val = (double)u.v[e];
+            double wv = w * val;
+            acc[e] += wv;
+            if (WITH_S2) acc2[e] = fma(wv, val, acc2[e]);
+        }
+        p += X;
+    }
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) {
+        part_rho[split * X + x + e] = acc[e];
+        if (WITH_S2) part_s2[split * X + x + e] = acc2[e];
+    }
+}
+
+// rho[x] = -sum_split part_rho[split][x] (fixed order);  s2[x] = +sum_split part_s2[split][x]
+__global__ void vsum_final_kernel(const double *__restrict__ part_rho,
+                                  const double *__restrict__ part_s2, long X, int splits,
+                                  double *__restrict__ rho, double *__restrict__ rho_copy,
+                                  double *__restrict__ s2) {
+    long x = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= X) return;
+    double a = 0.0, b = 0.0;
+    for (int s = 0; s < splits; ++s) {
+        a += part_rho[(long)s * X + x];
+        if (part_s2) b += part_s2[(long)s * X + x];
+    }
+    rho[x] = -a;
+    if (rho_copy) rho_copy[x] = -a;
+    if (s2) s2[x] = b;
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
+    return v;
+}
+
+// One block of 1024 threads.  out[0] = sum_x W_x (-rho[x]) (mass), out[1] = sum_x W_x s2[x]
+// (l2 squared), out[2] = 1/2 sum_x W_x sum_a E_a[x]^2 (electric energy).
+__global__ void __launch_bounds__(1024)
+scalars_kernel(const double *__restrict__ rho, const double *__restrict__ s2,
+               const double *__restrict__ E, const double *__restrict__ Wx, long X, int dx,
+               double *__restrict__ out) {
+    __shared__ double sm[3][32];
+    double a = 0.0, b = 0.0, c = 0.0;
+    for (long x = threadIdx.x; x < X; x += blockDim.x) {
+        double w = Wx[x];
+        a -= w * rho[x];
+        b += w * s2[x];
+        double e2 = 0.0;
+        for (int d = 0; d < dx; ++d) { double e = E[(long)d * X + x]; e2 = fma(e, e, e2); }
+        c += w * e2;
+    }
+    a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { sm[0][wid] = a; sm[1][wid] = b; sm[2][wid] = c; }
+    __syncthreads();
+    if (wid == 0) {
+        a = sm[0][lane]; b = sm[1][lane]; c = sm[2][lane];
+        a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+        if (lane == 0) { out[0] = a; out[1] = b; out[2] = 0.5 * c; }
+    }
+}
+
+}  // namespace sldg

@@ -1,0 +1,605 @@
+// sldg.cu -- implementation of include/sldg.h: context, dispatch and the Strang step.
+// Every step of the path runs in the kernels of sweep.cuh / reduce.cuh / poisson.cuh; there is
+// no CPU fallback (a missing device or an uninstantiated (order, dtype) is an error).
+#include "../../include/sldg.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "fill.cuh"
+#include "poisson.cuh"
+#include "reduce.cuh"
+#include "sweep.cuh"
+#include "tables.hpp"
+
+using namespace sldg;
+
+namespace {
+char g_create_error[512] = "";
+}
+
+struct sldg_ctx {
+    int dx = 0, dv = 0, D = 0, o = 0;
+    sldg_dtype dtype = SLDG_F64;
+    size_t esize = 8;
+    int cells[SLDG_MAX_DIM] = {0};
+    long N[SLDG_MAX_DIM] = {0};
+    double lo[SLDG_MAX_DIM] = {0}, hi[SLDG_MAX_DIM] = {0}, h[SLDG_MAX_DIM] = {0};
+    long X = 1, V = 1, ndof = 1;
+    double xi[SLDG_MAX_ORDER] = {0}, w[SLDG_MAX_ORDER] = {0};
+    void *buf[2] = {nullptr, nullptr};
+    int cur = 0;
+    cudaStream_t stream = nullptr;
+    int sm_count = 148;
+
+    // device tables
+    double *d_coef = nullptr;          // A/B polynomial coefficients [2][o][o][2o]
+    double *d_coords[SLDG_MAX_DIM] = {nullptr};   // node coordinates per dimension
+    long tab_cap = 0;                  // capacity (entries) of the sweep tables
+    double *d_sigma = nullptr;         // [tab_cap]
+    int *d_m = nullptr;                // [tab_cap]
+    void *d_ab = nullptr;              // [2 o^2][tab_cap] of T
+    double *d_Wv = nullptr, *d_Wx = nullptr;      // quadrature weights over v-nodes / x-nodes
+    double *d_rho = nullptr, *d_s2 = nullptr, *d_E = nullptr;   // [X], [X], [dx][X]
+    int max_splits = 1;
+    double *d_part = nullptr;          // [2][max_splits][X]
+    double *d_scal = nullptr;          // [3]
+    // Poisson
+    long K[3] = {1, 1, 1}, Mmax[3] = {0, 0, 0}, KK = 1;
+    double2 *d_F[3] = {nullptr, nullptr, nullptr}, *d_G[3] = {nullptr, nullptr, nullptr};
+    double *d_t[4] = {nullptr, nullptr, nullptr, nullptr};   // complex scratch (re, im) x 2
+    double *d_gh[2] = {nullptr, nullptr};                    // g_hat (re, im) [KK]
+
+    bool have_rho = false, have_E = false;
+    unsigned long long launches = 0;
+    char err[512] = "";
+};
+
+namespace {
+
+int fail(sldg_ctx *c, int code, const char *fmt, ...) {
+    char *dst = c ? c->err : g_create_error;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(c, call)                                                                  \
+    do {                                                                                   \
+        cudaError_t e_ = (call);                                                           \
+        if (e_ != cudaSuccess)                                                             \
+            return fail((c), SLDG_ERR_CUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                        __FILE__, __LINE__);                                               \
+    } while (0)
+
+#define LAUNCH_CHECK(c)                                                                     \
+    do {                                                                                    \
+        (c)->launches++;                                                                    \
+        cudaError_t e_ = cudaGetLastError();                                                \
+        if (e_ != cudaSuccess)                                                              \
+            return fail((c), SLDG_ERR_CUDA, "kernel launch: %s (%s:%d)", cudaGetErrorString(e_), \
+                        __FILE__, __LINE__);                                                \
+    } while (0)
+
+inline long cdiv(long a, long b) { return (a + b - 1) / b; }
+
+template <typename P>
+cudaError_t dalloc(P **p, size_t count) {
+    return cudaMalloc((void **)p, (count ? count : 1) * sizeof(P));
+}
+
+void free_tables(sldg_ctx *c) {
+    cudaFree(c->d_coef);
+    for (int d = 0; d < SLDG_MAX_DIM; ++d) cudaFree(c->d_coords[d]);
+    cudaFree(c->d_sigma); cudaFree(c->d_m); cudaFree(c->d_ab);
+    cudaFree(c->d_Wv); cudaFree(c->d_Wx);
+    cudaFree(c->d_rho); cudaFree(c->d_s2); cudaFree(c->d_E);
+    cudaFree(c->d_part); cudaFree(c->d_scal);
+    for (int a = 0; a < 3; ++a) { cudaFree(c->d_F[a]); cudaFree(c->d_G[a]); }
+    for (int i = 0; i < 4; ++i) cudaFree(c->d_t[i]);
+    cudaFree(c->d_gh[0]); cudaFree(c->d_gh[1]);
+}
+
+void host_node_coords(const sldg_ctx *c, int d, std::vector<double> &out) {
+    out.resize(c->N[d]);
+    for (int i = 0; i < c->cells[d]; ++i)
+        for (int j = 0; j < c->o; ++j) out[(size_t)i * c->o + j] = c->lo[d] + ((double)i + c->xi[j]) * c->h[d];
+}
+
+}  // namespace
+
+extern "C" const char *sldg_last_error(const sldg_ctx *ctx) { return ctx ? ctx->err : g_create_error; }
+extern "C" size_t sldg_num_dofs(const sldg_ctx *ctx) { return ctx ? (size_t)ctx->ndof : 0; }
+extern "C" size_t sldg_num_x(const sldg_ctx *ctx) { return ctx ? (size_t)ctx->X : 0; }
+extern "C" unsigned long long sldg_launch_count(const sldg_ctx *ctx) { return ctx ? ctx->launches : 0; }
+extern "C" void *sldg_current(sldg_ctx *ctx) { return ctx ? ctx->buf[ctx->cur] : nullptr; }
+
+extern "C" int sldg_node_coords(const sldg_ctx *ctx, int dim, double *host_out) {
+    if (!ctx || !host_out || dim < 0 || dim >= ctx->D) return SLDG_ERR_ARG;
+    std::vector<double> c;
+    host_node_coords(ctx, dim, c);
+    memcpy(host_out, c.data(), c.size() * sizeof(double));
+    return SLDG_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// create / destroy
+// ------------------------------------------------------------------------------------------
+extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int order,
+                           const double *lo, const double *hi, sldg_dtype dtype, void *f_buf0,
+                           void *f_buf1, void *cuda_stream) {
+    if (!out) return fail(nullptr, SLDG_ERR_ARG, "sldg_create: out is NULL");
+    *out = nullptr;
+    if (dx < 1 || dx > 3 || dv < 1 || dv > 3 || dv < dx)
+        return fail(nullptr, SLDG_ERR_ARG, "sldg_create: need 1 <= dx <= dv <= 3 (got %d+%d)", dx, dv);
+    if (!cells || !lo || !hi || !f_buf0 || !f_buf1 || f_buf0 == f_buf1)
+        return fail(nullptr, SLDG_ERR_ARG, "sldg_create: null or aliased argument");
+    if (order < 1 || order > SLDG_MAX_ORDER)
+        return fail(nullptr, SLDG_ERR_UNSUPPORTED, "sldg_create: order %d not in 1..%d", order, SLDG_MAX_ORDER);
+    if (dtype != SLDG_F64 && dtype != SLDG_F32)
+        return fail(nullptr, SLDG_ERR_UNSUPPORTED, "sldg_create: unknown dtype %d", (int)dtype);
+    if (((uintptr_t)f_buf0 | (uintptr_t)f_buf1) & 15)
+        return fail(nullptr, SLDG_ERR_ARG, "sldg_create: f buffers must be 16-byte aligned");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)
+        return fail(nullptr, SLDG_ERR_CUDA, "sldg_create: no CUDA device (this library has no CPU path)");
+
+    sldg_ctx *c = new sldg_ctx();
+    c->dx = dx; c->dv = dv; c->D = dx + dv; c->o = order; c->dtype = dtype;
+    c->esize = dtype == SLDG_F64 ? 8 : 4;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->buf[0] = f_buf0; c->buf[1] = f_buf1;
+    for (int d = 0; d < c->D; ++d) {
+        if (cells[d] < 1 || !(hi[d] > lo[d])) {
+            delete c;
+            return fail(nullptr, SLDG_ERR_ARG, "sldg_create: bad cells/domain in dimension %d", d);
+        }
+        c->cells[d] = cells[d]; c->lo[d] = lo[d]; c->hi[d] = hi[d];
+        c->h[d] = (hi[d] - lo[d]) / cells[d];
+        c->N[d] = (long)cells[d] * order;
+        c->ndof *= c->N[d];
+        if (d < dx) c->X *= c->N[d]; else c->V *= c->N[d];
+    }
+    gauss_legendre_01(order, c->xi, c->w);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+
+#define CREATE_TRY(call)                                                                        \
+    do {                                                                                        \
+        cudaError_t e_ = (call);                                                                \
+        if (e_ != cudaSuccess) {                                                                \
+            fail(nullptr, SLDG_ERR_CUDA, "sldg_create: %s: %s", #call, cudaGetErrorString(e_)); \
+            free_tables(c); delete c; return SLDG_ERR_CUDA;                                     \
+        }                                                                                       \
+    } while (0)
+
+    // A/B polynomial coefficients
+    std::vector<double> coef = ab_polynomial_coefficients(order);
+    CREATE_TRY(dalloc(&c->d_coef, coef.size()));
+    CREATE_TRY(cudaMemcpy(c->d_coef, coef.data(), coef.size() * sizeof(double), cudaMemcpyHostToDevice));
+
+    // node coordinates, sweep tables
+    long maxN = 0;
+    for (int d = 0; d < c->D; ++d) {
+        std::vector<double> cc;
+        host_node_coords(c, d, cc);
+        CREATE_TRY(dalloc(&c->d_coords[d], cc.size()));
+        CREATE_TRY(cudaMemcpy(c->d_coords[d], cc.data(), cc.size() * sizeof(double), cudaMemcpyHostToDevice));
+        if (c->N[d] > maxN) maxN = c->N[d];
+    }
+    c->tab_cap = c->X > maxN ? c->X : maxN;
+    CREATE_TRY(dalloc(&c->d_sigma, c->tab_cap));
+    CREATE_TRY(dalloc(&c->d_m, c->tab_cap));
+    CREATE_TRY(cudaMalloc(&c->d_ab, (size_t)2 * order * order * c->tab_cap * c->esize));
+
+    // quadrature weights W_v = prod_a h_va w_ja (v_1 fastest), W_x likewise
+    {
+        std::vector<double> Wv(c->V), Wx(c->X);
+        for (long v = 0; v < c->V; ++v) {
+            long rem = v; double W = 1.0;
+            for (int a = 0; a < dv; ++a) {
+                long p = rem % c->N[dx + a]; rem /= c->N[dx + a];
+                W *= c->h[dx + a] * c->w[p % order];
+            }
+            Wv[v] = W;
+        }
+        for (long x = 0; x < c->X; ++x) {
+            long rem = x; double W = 1.0;
+            for (int a = 0; a < dx; ++a) {
+                long p = rem % c->N[a]; rem /= c->N[a];
+                W *= c->h[a] * c->w[p % order];
+            }
+            Wx[x] = W;
+        }
+        CREATE_TRY(dalloc(&c->d_Wv, Wv.size()));
+        CREATE_TRY(dalloc(&c->d_Wx, Wx.size()));
+        CREATE_TRY(cudaMemcpy(c->d_Wv, Wv.data(), Wv.size() * sizeof(double), cudaMemcpyHostToDevice));
+        CREATE_TRY(cudaMemcpy(c->d_Wx, Wx.data(), Wx.size() * sizeof(double), cudaMemcpyHostToDevice));
+    }
+    CREATE_TRY(dalloc(&c->d_rho, c->X));
+    CREATE_TRY(dalloc(&c->d_s2, c->X));
+    CREATE_TRY(dalloc(&c->d_E, c->X * dx));
+    CREATE_TRY(cudaMemset(c->d_E, 0, c->X * dx * sizeof(double)));
+    CREATE_TRY(cudaMemset(c->d_s2, 0, c->X * sizeof(double)));
+    CREATE_TRY(dalloc(&c->d_scal, 3));
+    {
+        // enough v-splits that X/VEC * splits threads fill the machine (about 2 waves of 2048/SM)
+        long target = (long)c->sm_count * 2048 * 2;
+        long per = c->X / 2 > 0 ? c->X / 2 : 1;
+        long s = cdiv(target, per);
+        long smax = c->V / 16 > 0 ? c->V / 16 : 1;
+        if (s > smax) s = smax;
+        if (s < 1) s = 1;
+        if (s > 1024) s = 1024;
+        c->max_splits = (int)s;
+        CREATE_TRY(dalloc(&c->d_part, (size_t)2 * c->max_splits * c->X));
+    }
+
+    // Poisson: dense DFT matrices per x-dimension (D:R6)
+    {
+        const double PI = 3.14159265358979323846264338327950288;
+        long big = c->X;
+        for (int a = 0; a < dx; ++a) {
+            c->Mmax[a] = (c->cells[a] - 1) / 2;
+            c->K[a] = 2 * c->Mmax[a] + 1;
+            c->KK *= c->K[a];
+        }
+        for (int a = 0; a < dx; ++a) {
+            long Na = c->N[a], Ka = c->K[a];
+            double L = c->hi[a] - c->lo[a];
+            std::vector<double> cc;
+            host_node_coords(c, a, cc);
+            std::vector<double2> F((size_t)Ka * Na), G((size_t)Na * Ka);
+            for (long r = 0; r < Ka; ++r) {
+                double k = 2.0 * PI * (double)(r - c->Mmax[a]) / L;
+                for (long p = 0; p < Na; ++p) {
+                    double ph = k * cc[p];
+                    double wq = c->w[p % order] * c->h[a] / L;
+                    F[(size_t)r * Na + p] = make_double2(wq * cos(ph), -wq * sin(ph));
+                    G[(size_t)p * Ka + r] = make_double2(cos(ph), sin(ph));
+                }
+            }
+            CREATE_TRY(dalloc(&c->d_F[a], F.size()));
+            CREATE_TRY(dalloc(&c->d_G[a], G.size()));
+            CREATE_TRY(cudaMemcpy(c->d_F[a], F.data(), F.size() * sizeof(double2), cudaMemcpyHostToDevice));
+            CREATE_TRY(cudaMemcpy(c->d_G[a], G.data(), G.size() * sizeof(double2), cudaMemcpyHostToDevice));
+        }
+        for (int i = 0; i < 4; ++i) CREATE_TRY(dalloc(&c->d_t[i], big));
+        CREATE_TRY(dalloc(&c->d_gh[0], c->KK));
+        CREATE_TRY(dalloc(&c->d_gh[1], c->KK));
+    }
+#undef CREATE_TRY
+    *out = c;
+    return SLDG_OK;
+}
+
+extern "C" int sldg_destroy(sldg_ctx *ctx) {
+    if (!ctx) return SLDG_ERR_ARG;
+    cudaStreamSynchronize(ctx->stream);
+    free_tables(ctx);
+    delete ctx;
+    return SLDG_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// f in / out
+// ------------------------------------------------------------------------------------------
+extern "C" int sldg_set_initial(sldg_ctx *c, const void *src, int is_device) {
+    if (!c || !src) return SLDG_ERR_ARG;
+    size_t bytes = (size_t)c->ndof * c->esize;
+    CUDA_TRY(c, cudaMemcpyAsync(c->buf[c->cur], src, bytes,
+                                is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    if (!is_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->have_rho = false;
+    return SLDG_OK;
+}
+
+extern "C" int sldg_get_f(sldg_ctx *c, void *dst, int is_device) {
+    if (!c || !dst) return SLDG_ERR_ARG;
+    size_t bytes = (size_t)c->ndof * c->esize;
+    CUDA_TRY(c, cudaMemcpyAsync(dst, c->buf[c->cur], bytes,
+                                is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+    if (!is_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return SLDG_OK;
+}
+
+extern "C" int sldg_fill_uniform(sldg_ctx *c, unsigned long long seed, unsigned tag) {
+    if (!c) return SLDG_ERR_ARG;
+    int blocks = c->sm_count * 8;
+    if (c->dtype == SLDG_F64)
+        fill_uniform_kernel<double><<<blocks, 256, 0, c->stream>>>((double *)c->buf[c->cur], c->ndof, seed, tag);
+    else
+        fill_uniform_kernel<float><<<blocks, 256, 0, c->stream>>>((float *)c->buf[c->cur], c->ndof, seed, tag);
+    LAUNCH_CHECK(c);
+    c->have_rho = false;
+    return SLDG_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// sweeps: a-1 (assemble) + a-2 (translate), d_sigma[0..count) already filled on the stream
+// ------------------------------------------------------------------------------------------
+namespace {
+
+template <typename T, int O, int VEC, bool QV>
+void launch_strided(sldg_ctx *c, const T *in, T *out, long inner, int n, long outer, long count,
+                    long qdiv, long qmod) {
+    constexpr int UB = (O <= 3) ? 4 : 2;
+    long lines_v = outer * (inner / VEC);
+    // split lines into segments only when there are too few of them to fill the machine
+    long target = (long)c->sm_count * 2048;
+    int nseg = 1;
+    if (lines_v < target) {
+        nseg = (int)cdiv(target, lines_v);
+        int maxseg = n / 4 > 0 ? n / 4 : 1;
+        if (nseg > maxseg) nseg = maxseg;
+    }
+    int cps = (int)cdiv(n, nseg);
+    nseg = (int)cdiv(n, cps);
+    long threads = lines_v * nseg;
+    int block = 256;
+    long blocks = cdiv(threads, block);
+    sweep_strided_kernel<T, O, VEC, QV, UB><<<(unsigned)blocks, block, 0, c->stream>>>(
+        in, out, inner, n, outer, nseg, cps, c->d_m, (const T *)c->d_ab, count, qdiv, qmod, c->X);
+}
+
+template <typename T, int O>
+int run_sweep_t(sldg_ctx *c, int dim, long count) {
+    const int n = c->cells[dim];
+    const T *in = (const T *)c->buf[c->cur];
+    T *out = (T *)c->buf[c->cur ^ 1];
+    // a-1
+    {
+        int block = 128;
+        size_t sh = (size_t)2 * O * O * 2 * O * sizeof(double);
+        assemble_ab_kernel<T><<<(unsigned)cdiv(count, block), block, sh, c->stream>>>(
+            c->d_sigma, count, O, n, c->d_coef, c->d_m, (T *)c->d_ab);
+        LAUNCH_CHECK(c);
+    }
+    long inner = 1, outer = 1;
+    for (int d = 0; d < dim; ++d) inner *= c->N[d];
+    for (int d = dim + 1; d < c->D; ++d) outer *= c->N[d];
+    if (dim == 0) {
+        // lines sharing a shift: q = (line / qdiv) % N_{v_1}, qdiv = prod_{1<=d<dx} N_d
+        long qdiv = 1;
+        for (int d = 1; d < c->dx; ++d) qdiv *= c->N[d];
+        long ngroups = outer / qdiv;
+        long cpg = qdiv * n;                       // cells per group
+        int block = 256;
+        int cpb = 2048;                            // cells per block
+        if (cpg < cpb) { cpb = (int)cpg; if (cpb < block) block = (int)(cdiv(cpb, 32) * 32); }
+        int bpg = (int)cdiv(cpg, cpb);
+        sweep_x1_kernel<T, O><<<(unsigned)(ngroups * bpg), block, 0, c->stream>>>(
+            in, out, n, ngroups, cpg, cpb, bpg, c->d_m, (const T *)c->d_ab, count, c->N[c->dx]);
+    } else if (dim < c->dx) {
+        const int dep = c->dx + dim;
+        long qdiv = 1;
+        for (int d = dim + 1; d < dep; ++d) qdiv *= c->N[d];
+        const long qmod = c->N[dep];
+        constexpr int VMAX = 16 / (int)sizeof(T);
+        if (inner % VMAX == 0) launch_strided<T, O, VMAX, false>(c, in, out, inner, n, outer, count, qdiv, qmod);
+        else if (inner % 2 == 0) launch_strided<T, O, 2, false>(c, in, out, inner, n, outer, count, qdiv, qmod);
+        else launch_strided<T, O, 1, false>(c, in, out, inner, n, outer, count, qdiv, qmod);
+    } else {
+        launch_strided<T, O, 1, true>(c, in, out, inner, n, outer, count, 1, 1);
+    }
+    LAUNCH_CHECK(c);
+    c->cur ^= 1;
+    c->have_rho = false;
+    return SLDG_OK;
+}
+
+template <typename T>
+int run_sweep_o(sldg_ctx *c, int dim, long count) {
+    switch (c->o) {
+    case 1: return run_sweep_t<T, 1>(c, dim, count);
+    case 2: return run_sweep_t<T, 2>(c, dim, count);
+    case 3: return run_sweep_t<T, 3>(c, dim, count);
+    case 4: return run_sweep_t<T, 4>(c, dim, count);
+    }
+    return fail(c, SLDG_ERR_UNSUPPORTED, "order %d not instantiated", c->o);
+}
+
+int run_sweep(sldg_ctx *c, int dim, long count) {
+    return c->dtype == SLDG_F64 ? run_sweep_o<double>(c, dim, count) : run_sweep_o<float>(c, dim, count);
+}
+
+long sweep_count(const sldg_ctx *c, int dim) { return dim < c->dx ? c->N[c->dx + dim] : c->X; }
+
+}  // namespace
+
+extern "C" int sldg_translate(sldg_ctx *c, int dim, const double *shift, size_t count) {
+    if (!c || !shift || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
+    if ((long)count != sweep_count(c, dim))
+        return fail(c, SLDG_ERR_ARG, "sldg_translate: dim %d needs %ld shifts, got %zu", dim, sweep_count(c, dim), count);
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift, count * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));   // the host array may be reused by the caller
+    return run_sweep(c, dim, (long)count);
+}
+
+extern "C" int sldg_translate_dev(sldg_ctx *c, int dim, const double *shift, size_t count) {
+    if (!c || !shift || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
+    if ((long)count != sweep_count(c, dim))
+        return fail(c, SLDG_ERR_ARG, "sldg_translate_dev: dim %d needs %ld shifts, got %zu", dim, sweep_count(c, dim), count);
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift, count * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    return run_sweep(c, dim, (long)count);
+}
+
+extern "C" int sldg_advect(sldg_ctx *c, int dim, double dt) {
+    if (!c || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
+    long count = sweep_count(c, dim);
+    int block = 256;
+    if (dim < c->dx) {
+        int va = c->dx + dim;
+        sigma_from_coords_kernel<<<(unsigned)cdiv(count, block), block, 0, c->stream>>>(
+            c->d_coords[va], count, dt, c->h[dim], c->d_sigma);
+    } else {
+        int a = dim - c->dx;
+        if (a >= c->dx) return fail(c, SLDG_ERR_ARG, "sldg_advect: v_%d has no field component (dx = %d)", a + 1, c->dx);
+        if (!c->have_E) return fail(c, SLDG_ERR_STATE, "sldg_advect: no E stored (call sldg_poisson_E or sldg_set_E)");
+        sigma_from_E_kernel<<<(unsigned)cdiv(count, block), block, 0, c->stream>>>(
+            c->d_E + (long)a * c->X, count, dt, c->h[dim], c->d_sigma);
+    }
+    LAUNCH_CHECK(c);
+    return run_sweep(c, dim, count);
+}
+
+// ------------------------------------------------------------------------------------------
+// a-3 rho, a-4 Poisson, a-5 step, a-6 diagnostics
+// ------------------------------------------------------------------------------------------
+namespace {
+
+template <typename T, int VEC, bool S2>
+void launch_vsum(sldg_ctx *c, int splits, long vps) {
+    int block = 128;
+    long xv = c->X / VEC;
+    if (xv < block) block = (int)(cdiv(xv, 32) * 32);
+    dim3 grid((unsigned)cdiv(xv, block), (unsigned)splits);
+    vsum_partial_kernel<T, VEC, S2, 8><<<grid, block, 0, c->stream>>>(
+        (const T *)c->buf[c->cur], c->X, c->V, vps, c->d_Wv, c->d_part,
+        c->d_part + (size_t)c->max_splits * c->X);
+}
+
+template <typename T, bool S2>
+int run_vsum(sldg_ctx *c, double *rho_copy) {
+    constexpr int VMAX = 16 / (int)sizeof(T);
+    int vec = (c->X % VMAX == 0) ? VMAX : ((c->X % 2 == 0) ? 2 : 1);
+    long target = (long)c->sm_count * 2048 * 2;
+    long s = cdiv(target, c->X / vec > 0 ? c->X / vec : 1);
+    if (s > c->max_splits) s = c->max_splits;
+    if (s < 1) s = 1;
+    long vps = cdiv(c->V, s);
+    int splits = (int)cdiv(c->V, vps);
+    if (vec == VMAX) launch_vsum<T, VMAX, S2>(c, splits, vps);
+    else if (vec == 2) launch_vsum<T, 2, S2>(c, splits, vps);
+    else launch_vsum<T, 1, S2>(c, splits, vps);
+    LAUNCH_CHECK(c);
+    int block = 256;
+    vsum_final_kernel<<<(unsigned)cdiv(c->X, block), block, 0, c->stream>>>(
+        c->d_part, S2 ? c->d_part + (size_t)c->max_splits * c->X : nullptr, c->X, splits, c->d_rho,
+        rho_copy, S2 ? c->d_s2 : nullptr);
+    LAUNCH_CHECK(c);
+    c->have_rho = true;
+    return SLDG_OK;
+}
+
+int run_rho(sldg_ctx *c, double *rho_copy, bool with_s2) {
+    if (c->dtype == SLDG_F64)
+        return with_s2 ? run_vsum<double, true>(c, rho_copy) : run_vsum<double, false>(c, rho_copy);
+    return with_s2 ? run_vsum<float, true>(c, rho_copy) : run_vsum<float, false>(c, rho_copy);
+}
+
+// apply M (rows x cols) along dimension b of a complex tensor with extents shape[] (index 0 fastest)
+template <bool IN_REAL, bool OUT_REAL>
+int apply_along(sldg_ctx *c, const double *in_re, const double *in_im, long *shape, int nd, int b,
+                const double2 *M, long rows, double *out_re, double *out_im) {
+    long inner = 1, outer = 1, cols = shape[b];
+    for (int d = 0; d < b; ++d) inner *= shape[d];
+    for (int d = b + 1; d < nd; ++d) outer *= shape[d];
+    long total = outer * rows * inner;
+    int block = 128;
+    cplx_apply_kernel<IN_REAL, OUT_REAL><<<(unsigned)cdiv(total, block), block, 0, c->stream>>>(
+        in_re, in_im, outer, cols, inner, M, rows, out_re, out_im);
+    LAUNCH_CHECK(c);
+    shape[b] = rows;
+    return SLDG_OK;
+}
+
+int run_poisson(sldg_ctx *c, double *E_copy) {
+    const double PI = 3.14159265358979323846264338327950288;
+    const int dx = c->dx;
+    long shape[3] = {1, 1, 1};
+    for (int a = 0; a < dx; ++a) shape[a] = c->N[a];
+    // forward transform of rho + 1, one dimension at a time
+    const double *ir = c->d_rho, *ii = nullptr;
+    int rc;
+    for (int a = 0; a < dx; ++a) {
+        double *orr = (a == dx - 1) ? c->d_gh[0] : c->d_t[(a & 1) * 2];
+        double *oi = (a == dx - 1) ? c->d_gh[1] : c->d_t[(a & 1) * 2 + 1];
+        if (a == 0) rc = apply_along<true, false>(c, ir, ii, shape, dx, a, c->d_F[a], c->K[a], orr, oi);
+        else rc = apply_along<false, false>(c, ir, ii, shape, dx, a, c->d_F[a], c->K[a], orr, oi);
+        if (rc) return rc;
+        ir = orr; ii = oi;
+    }
+    double kf[3] = {0, 0, 0};
+    for (int a = 0; a < dx; ++a) kf[a] = 2.0 * PI / (c->hi[a] - c->lo[a]);
+    for (int a = 0; a < dx; ++a) {
+        int block = 128;
+        poisson_scale_kernel<<<(unsigned)cdiv(c->KK, block), block, 0, c->stream>>>(
+            c->d_gh[0], c->d_gh[1], c->KK, dx, a, c->K[0], c->K[1], c->K[2], c->Mmax[0], c->Mmax[1],
+            c->Mmax[2], kf[0], kf[1], kf[2], c->d_t[0], c->d_t[1]);
+        LAUNCH_CHECK(c);
+        for (int b = 0; b < dx; ++b) shape[b] = c->K[b];
+        const double *sr = c->d_t[0], *si = c->d_t[1];
+        for (int b = 0; b < dx; ++b) {
+            bool last = (b == dx - 1);
+            double *orr = last ? c->d_E + (long)a * c->X : c->d_t[((b + 1) & 1) * 2];
+            double *oi = last ? nullptr : c->d_t[((b + 1) & 1) * 2 + 1];
+            if (last) rc = apply_along<false, true>(c, sr, si, shape, dx, b, c->d_G[b], c->N[b], orr, oi);
+            else rc = apply_along<false, false>(c, sr, si, shape, dx, b, c->d_G[b], c->N[b], orr, oi);
+            if (rc) return rc;
+            sr = orr; si = oi;
+        }
+    }
+    c->have_E = true;
+    if (E_copy)
+        CUDA_TRY(c, cudaMemcpyAsync(E_copy, c->d_E, (size_t)dx * c->X * sizeof(double),
+                                    cudaMemcpyDeviceToDevice, c->stream));
+    return SLDG_OK;
+}
+
+}  // namespace
+
+extern "C" int sldg_compute_rho(sldg_ctx *c, double *rho_out) {
+    if (!c) return SLDG_ERR_ARG;
+    return run_rho(c, rho_out, false);
+}
+
+extern "C" int sldg_poisson_E(sldg_ctx *c, double *E_out) {
+    if (!c) return SLDG_ERR_ARG;
+    if (!c->have_rho) return fail(c, SLDG_ERR_STATE, "sldg_poisson_E: rho of the current f not computed");
+    return run_poisson(c, E_out);
+}
+
+extern "C" int sldg_set_E(sldg_ctx *c, const double *E, int is_device) {
+    if (!c || !E) return SLDG_ERR_ARG;
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_E, E, (size_t)c->dx * c->X * sizeof(double),
+                                is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    if (!is_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->have_E = true;
+    return SLDG_OK;
+}
+
+extern "C" int sldg_step(sldg_ctx *c, double dt) {
+    if (!c) return SLDG_ERR_ARG;
+    int rc;
+    for (int a = 0; a < c->dx; ++a) if ((rc = sldg_advect(c, a, 0.5 * dt))) return rc;
+    if ((rc = run_rho(c, nullptr, false))) return rc;
+    if ((rc = run_poisson(c, nullptr))) return rc;
+    for (int a = 0; a < c->dx; ++a) if ((rc = sldg_advect(c, c->dx + a, dt))) return rc;
+    for (int a = 0; a < c->dx; ++a) if ((rc = sldg_advect(c, a, 0.5 * dt))) return rc;
+    return SLDG_OK;
+}
+
+extern "C" int sldg_diagnostics(sldg_ctx *c, double *mass, double *l2, double *ee) {
+    if (!c) return SLDG_ERR_ARG;
+    int rc;
+    if ((rc = run_rho(c, nullptr, true))) return rc;
+    if ((rc = run_poisson(c, nullptr))) return rc;
+    scalars_kernel<<<1, 1024, 0, c->stream>>>(c->d_rho, c->d_s2, c->d_E, c->d_Wx, c->X, c->dx, c->d_scal);
+    LAUNCH_CHECK(c);
+    double h[3];
+    CUDA_TRY(c, cudaMemcpyAsync(h, c->d_scal, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    if (mass) *mass = h[0];
+    if (l2) *l2 = sqrt(h[1]);
+    if (ee) *ee = h[2];
+    return SLDG_OK;
+}

@@ -1,0 +1,194 @@
+"""Python binding of the C-ABI library (include/sldg.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libsldg.so.  PyTorch provides device
+memory and the stream.  Importing this module loads libsldg.so and raises if it has not
+been built; there is no CPU fallback.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+SLDG_F64, SLDG_F32 = 0, 1
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsldg.so")
+
+EXPORTS = [
+    "sldg_create", "sldg_destroy", "sldg_last_error", "sldg_num_dofs", "sldg_num_x",
+    "sldg_node_coords", "sldg_set_initial", "sldg_get_f", "sldg_current", "sldg_fill_uniform",
+    "sldg_translate", "sldg_translate_dev", "sldg_advect", "sldg_compute_rho", "sldg_poisson_E",
+    "sldg_set_E", "sldg_step", "sldg_diagnostics", "sldg_launch_count",
+]
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "libsldg.so is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+            "(or python -m paper_1907_08316_b200.build).  There is no CPU fallback.")
+    lib = C.CDLL(LIB_PATH)
+    vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
+    lib.sldg_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, ip, C.c_int, dp, dp, C.c_int, vp, vp, vp]
+    lib.sldg_destroy.argtypes = [vp]
+    lib.sldg_last_error.argtypes = [vp]
+    lib.sldg_last_error.restype = C.c_char_p
+    lib.sldg_num_dofs.argtypes = [vp]
+    lib.sldg_num_dofs.restype = C.c_size_t
+    lib.sldg_num_x.argtypes = [vp]
+    lib.sldg_num_x.restype = C.c_size_t
+    lib.sldg_node_coords.argtypes = [vp, C.c_int, dp]
+    lib.sldg_set_initial.argtypes = [vp, vp, C.c_int]
+    lib.sldg_get_f.argtypes = [vp, vp, C.c_int]
+    lib.sldg_current.argtypes = [vp]
+    lib.sldg_current.restype = vp
+    lib.sldg_fill_uniform.argtypes = [vp, C.c_ulonglong, C.c_uint]
+    lib.sldg_translate.argtypes = [vp, C.c_int, dp, C.c_size_t]
+    lib.sldg_translate_dev.argtypes = [vp, C.c_int, vp, C.c_size_t]
+    lib.sldg_advect.argtypes = [vp, C.c_int, C.c_double]
+    lib.sldg_compute_rho.argtypes = [vp, vp]
+    lib.sldg_poisson_E.argtypes = [vp, vp]
+    lib.sldg_set_E.argtypes = [vp, vp, C.c_int]
+    lib.sldg_step.argtypes = [vp, C.c_double]
+    lib.sldg_diagnostics.argtypes = [vp, dp, dp, dp]
+    lib.sldg_launch_count.argtypes = [vp]
+    lib.sldg_launch_count.restype = C.c_ulonglong
+    return lib
+
+
+_lib = _load()
+
+
+class SldgError(RuntimeError):
+    pass
+
+
+class Sldg:
+    """One solver context.  Allocates the two f buffers as torch CUDA tensors (caller-owned
+    memory in the sense of sldg.h) and forwards every call to the library."""
+
+    def __init__(self, dx, dv, cells, order, lo, hi, dtype="f64", device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise SldgError("no CUDA device: the SLDG library has no CPU path")
+        self.torch = torch
+        self.dx, self.dv, self.order = int(dx), int(dv), int(order)
+        D = self.dx + self.dv
+        self.cells = tuple(int(c) for c in cells)
+        self.N = tuple(c * self.order for c in self.cells)
+        self.X = int(np.prod(self.N[: self.dx]))
+        self.ndof = int(np.prod(self.N))
+        self.dtype = {"f64": SLDG_F64, "f32": SLDG_F32}[dtype]
+        self.tdtype = torch.float64 if dtype == "f64" else torch.float32
+        self.npdtype = np.float64 if dtype == "f64" else np.float32
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.buf = [torch.empty(self.ndof, dtype=self.tdtype, device=self.device) for _ in range(2)]
+        cells_a = (C.c_int * D)(*self.cells)
+        lo_a = (C.c_double * D)(*[float(x) for x in lo])
+        hi_a = (C.c_double * D)(*[float(x) for x in hi])
+        h = C.c_void_p()
+        rc = _lib.sldg_create(C.byref(h), self.dx, self.dv, cells_a, self.order, lo_a, hi_a, self.dtype,
+                              self.buf[0].data_ptr(), self.buf[1].data_ptr(), self.stream.cuda_stream)
+        if rc != 0:
+            raise SldgError("sldg_create failed (%d): %s" % (rc, _lib.sldg_last_error(None).decode()))
+        self.h = h
+
+    @classmethod
+    def from_config(cls, cfg, dtype="f64", **kw):
+        return cls(cfg.dx, cfg.dv, cfg.cells, cfg.order, cfg.lo, cfg.hi, dtype=dtype, **kw)
+
+    def _chk(self, rc, what):
+        if rc != 0:
+            raise SldgError("%s failed (%d): %s" % (what, rc, _lib.sldg_last_error(self.h).decode()))
+
+    def close(self):
+        if getattr(self, "h", None):
+            _lib.sldg_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- data in / out
+    def node_coords(self, dim):
+        out = np.zeros(self.N[dim], dtype=np.float64)
+        self._chk(_lib.sldg_node_coords(self.h, dim, out.ctypes.data_as(C.POINTER(C.c_double))), "node_coords")
+        return out
+
+    def set_initial(self, f):
+        """f: numpy array (host) or torch CUDA tensor, N values of the context's dtype."""
+        if isinstance(f, np.ndarray):
+            f = np.ascontiguousarray(f, dtype=self.npdtype).reshape(-1)
+            assert f.size == self.ndof
+            self._chk(_lib.sldg_set_initial(self.h, f.ctypes.data, 0), "set_initial")
+        elif f.is_cuda:
+            assert f.dtype == self.tdtype and f.numel() == self.ndof and f.is_contiguous()
+            self._chk(_lib.sldg_set_initial(self.h, f.data_ptr(), 1), "set_initial")
+        else:   # host torch tensor (e.g. pinned)
+            assert f.dtype == self.tdtype and f.numel() == self.ndof and f.is_contiguous()
+            self._chk(_lib.sldg_set_initial(self.h, f.data_ptr(), 0), "set_initial")
+
+    def get_f(self, out=None):
+        """Copy f to host: into `out` (numpy or host torch tensor) or a new numpy array."""
+        if out is None:
+            out = np.empty(self.ndof, dtype=self.npdtype)
+        ptr = out.ctypes.data if isinstance(out, np.ndarray) else out.data_ptr()
+        self._chk(_lib.sldg_get_f(self.h, ptr, 0), "get_f")
+        return out
+
+    def current(self):
+        """The torch tensor (view of the caller-owned buffer) that holds f now."""
+        p = _lib.sldg_current(self.h)
+        return self.buf[0] if p == self.buf[0].data_ptr() else self.buf[1]
+
+    def fill_uniform(self, seed, tag=0):
+        self._chk(_lib.sldg_fill_uniform(self.h, int(seed), int(tag)), "fill_uniform")
+
+    # ---- the path
+    def translate(self, dim, shift_cells):
+        if isinstance(shift_cells, np.ndarray):
+            s = np.ascontiguousarray(shift_cells, dtype=np.float64).reshape(-1)
+            self._chk(_lib.sldg_translate(self.h, dim, s.ctypes.data_as(C.POINTER(C.c_double)), s.size), "translate")
+        else:
+            assert shift_cells.is_cuda and shift_cells.dtype == self.torch.float64 and shift_cells.is_contiguous()
+            self._chk(_lib.sldg_translate_dev(self.h, dim, shift_cells.data_ptr(), shift_cells.numel()), "translate_dev")
+
+    def advect(self, dim, dt):
+        self._chk(_lib.sldg_advect(self.h, dim, float(dt)), "advect")
+
+    def compute_rho(self):
+        rho = self.torch.empty(self.X, dtype=self.torch.float64, device=self.device)
+        self._chk(_lib.sldg_compute_rho(self.h, rho.data_ptr()), "compute_rho")
+        return rho
+
+    def poisson_E(self):
+        E = self.torch.empty((self.dx, self.X), dtype=self.torch.float64, device=self.device)
+        self._chk(_lib.sldg_poisson_E(self.h, E.data_ptr()), "poisson_E")
+        return E
+
+    def set_E(self, E):
+        if isinstance(E, np.ndarray):
+            E = np.ascontiguousarray(E, dtype=np.float64).reshape(-1)
+            assert E.size == self.dx * self.X
+            self._chk(_lib.sldg_set_E(self.h, E.ctypes.data, 0), "set_E")
+        else:
+            assert E.is_cuda and E.dtype == self.torch.float64 and E.numel() == self.dx * self.X
+            self._chk(_lib.sldg_set_E(self.h, E.data_ptr(), 1), "set_E")
+
+    def step(self, dt):
+        self._chk(_lib.sldg_step(self.h, float(dt)), "step")
+
+    def diagnostics(self):
+        m, l2, ee = C.c_double(), C.c_double(), C.c_double()
+        self._chk(_lib.sldg_diagnostics(self.h, C.byref(m), C.byref(l2), C.byref(ee)), "diagnostics")
+        return m.value, l2.value, ee.value
+
+    def launch_count(self):
+        return int(_lib.sldg_launch_count(self.h))

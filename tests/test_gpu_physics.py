@@ -1,0 +1,145 @@
+"""-m gpu: rho, Poisson, Strang step and diagnostics of the CUDA library against the CPU oracle
+on the BASELINE.json configs (configs 1-2 at full size, 3 and 5 as reduced twins here; the
+full-size launch configurations are covered in test_gpu_fullsize.py)."""
+import numpy as np
+import pytest
+
+from paper_1907_08316_b200 import workloads as W
+from tests.gpu_util import NPDT, TOL, make_solver, rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+def _grid(oracle, cfg):
+    return oracle.Grid(cfg.dx, cfg.dv, cfg.cells, cfg.order, cfg.lo, cfg.hi)
+
+
+def _coords(oracle, cfg):
+    g = _grid(oracle, cfg)
+    return [g.coords(d) for d in range(cfg.dx + cfg.dv)]
+
+
+def test_node_coords_match_oracle_to_one_ulp(oracle):
+    for o in (1, 2, 3, 4):
+        cfg = W.Config("c", 1, 1, (7, 5), o, (0.0, -6.0), (4 * np.pi, 6.0))
+        s = make_solver(cfg, "f64")
+        for d in range(2):
+            a, b = s.node_coords(d), _grid(oracle, cfg).coords(d)
+            assert np.max(np.abs(a - b)) <= 2 * np.spacing(np.max(np.abs(b)))
+        s.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(1, 1, (9, 7)), (2, 2, (6, 5, 4, 7)), (3, 3, (4, 3, 5, 3, 4, 3)),
+                                   (1, 2, (8, 5, 4)), (2, 3, (5, 4, 3, 4, 3))])
+def test_rho_poisson_diagnostics(oracle, shape, dtype):
+    dx, dv, cells = shape
+    o = 3 if dx < 3 else 2
+    lo = (0.0,) * dx + (-4.0,) * dv
+    hi = tuple(2 * np.pi * (1 + 0.5 * a) for a in range(dx)) + (4.0,) * dv
+    cfg = W.Config("r", dx, dv, cells, o, lo, hi)
+    rng = np.random.default_rng(5)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
+    g = _grid(oracle, cfg)
+    s = make_solver(cfg, dtype)
+    s.set_initial(f0)
+    rho = s.compute_rho().cpu().numpy()
+    rho_ref = g.rho(f0)
+    assert rel_err(rho, rho_ref) <= 1e-13
+    E = s.poisson_E().cpu().numpy()
+    E_ref = g.poisson_E(rho_ref)
+    assert rel_err(E, E_ref) <= 1e-12
+    m, l2, ee = s.diagnostics()
+    mr, l2r, eer = g.diagnostics(f0)
+    assert abs(m - mr) <= 1e-13 * abs(mr)
+    assert abs(l2 - l2r) <= 1e-13 * abs(l2r)
+    assert abs(ee - eer) <= 1e-11 * abs(eer)
+    s.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_advect_physics_shifts(oracle, dtype):
+    """sldg_advect derives sigma from the v-node coordinates / from E exactly as D:O3, D:R4."""
+    cfg = W.CONFIG3.scaled((6, 5, 8, 7))
+    g = _grid(oracle, cfg)
+    f0 = W.initial_state(cfg, _coords(oracle, cfg), NPDT[dtype])
+    rng = np.random.default_rng(11)
+    E = rng.uniform(-2.0, 2.0, (cfg.dx, cfg.X))
+    s = make_solver(cfg, dtype)
+    s.set_initial(f0)
+    s.set_E(E)
+    ref = f0.copy()
+    for dim, tau in ((0, 0.37), (1, 0.21), (2, 0.4), (3, 0.15)):
+        s.advect(dim, tau)
+        g.advect(ref, dim, tau, E if dim >= cfg.dx else None)
+        assert rel_err(s.get_f(), ref) <= TOL[dtype], dim
+    s.close()
+
+
+def _run_config(oracle, cfg, dtype, steps):
+    g = _grid(oracle, cfg)
+    f0 = W.initial_state(cfg, _coords(oracle, cfg), NPDT[dtype])
+    s = make_solver(cfg, dtype)
+    s.set_initial(f0)
+    ref = f0.copy()
+    tr_gpu, tr_ref = [s.diagnostics()], [g.diagnostics(ref)]
+    for _ in range(steps):
+        s.step(cfg.dt)
+        g.step(ref, cfg.dt)
+        tr_gpu.append(s.diagnostics())
+        tr_ref.append(g.diagnostics(ref))
+    got = s.get_f()
+    s.close()
+    return got, ref, np.array(tr_gpu), np.array(tr_ref)
+
+
+def _check_traces(tr_gpu, tr_ref, tol):
+    # D:R11: |ee_gpu - ee_cpu| <= tol * max_n ee_cpu; mass and l2 relative
+    assert np.max(np.abs(tr_gpu[:, 2] - tr_ref[:, 2])) <= tol * np.max(tr_ref[:, 2])
+    assert np.max(np.abs(tr_gpu[:, 0] - tr_ref[:, 0])) <= tol * np.max(np.abs(tr_ref[:, 0]))
+    assert np.max(np.abs(tr_gpu[:, 1] - tr_ref[:, 1])) <= tol * np.max(tr_ref[:, 1])
+
+
+def landau_gamma(ee, dt):
+    """D:R14: slope of the line through the local maxima #2..#8 of a_n = 1/2 ln ee(t_n)."""
+    a = 0.5 * np.log(ee)
+    pk = [n for n in range(1, len(a) - 1) if a[n] > a[n - 1] and a[n] >= a[n + 1]]
+    pk = pk[1:8]
+    t = np.array(pk) * dt
+    return float(np.polyfit(t, a[pk], 1)[0])
+
+
+def test_config1_landau_1p1_full_run(oracle):
+    cfg = W.CONFIG1
+    got, ref, tg, tr = _run_config(oracle, cfg, "f64", cfg.steps)
+    assert rel_err(got, ref) <= TOL["f64"]
+    _check_traces(tg, tr, TOL["f64"])
+    # P5 mass conservation, P9 ee(0) closed form, P10 decay rate -- on the GPU trace itself
+    assert np.max(np.abs(tg[:, 0] - tg[0, 0])) <= 1e-13 * abs(tg[0, 0])
+    assert abs(tg[0, 2] - 0.25 * (cfg.eps / cfg.k) ** 2 * 4 * np.pi) <= 1e-7 * tg[0, 2]
+    gamma = landau_gamma(tg[:, 2], cfg.dt)
+    assert abs(gamma - (-0.1533)) <= 0.02 * 0.1533
+    assert np.all(np.diff(tg[:, 1]) <= 1e-14 * tg[0, 1])       # P8: l2 never increases
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config2_twostream_1p1_full_run(oracle, dtype):
+    cfg = W.CONFIG2
+    got, ref, tg, tr = _run_config(oracle, cfg, dtype, cfg.steps)
+    assert rel_err(got, ref) <= TOL[dtype]
+    _check_traces(tg, tr, TOL[dtype])
+
+
+def test_config3_reduced_twin(oracle):
+    cfg = W.CONFIG3.scaled((16, 16, 16, 16))
+    got, ref, tg, tr = _run_config(oracle, cfg, "f64", cfg.steps)
+    assert rel_err(got, ref) <= TOL["f64"]
+    _check_traces(tg, tr, TOL["f64"])
+    assert abs(tg[0, 2] - 2 * 0.25 * (cfg.eps / cfg.k) ** 2 * (4 * np.pi) ** 2) <= 1e-3 * tg[0, 2]
+
+
+def test_config5_reduced_twin(oracle):
+    cfg = W.CONFIG5.scaled((8, 8, 8, 8, 8, 8))
+    got, ref, tg, tr = _run_config(oracle, cfg, "f64", cfg.steps)
+    assert rel_err(got, ref) <= TOL["f64"]
+    _check_traces(tg, tr, TOL["f64"])

@@ -1,0 +1,121 @@
+"""-m gpu: the CUDA translation sweep (sldg_translate / sldg_advect) against the CPU oracle,
+element by element, on seeded inputs spanning several tiles and ragged tails."""
+import numpy as np
+import pytest
+
+from paper_1907_08316_b200 import workloads as W
+from tests.gpu_util import NPDT, TOL, dep_of, make_solver, rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+def _random_shifts(rng, count, kind):
+    if kind == "small":                    # |sigma| << 1 as in the physics v-sweeps
+        return rng.uniform(-0.3, 0.3, count)
+    if kind == "wide":                     # config-4 like
+        return rng.uniform(-3.5, 3.5, count)
+    if kind == "integer":                  # exact translation (P4)
+        return rng.integers(-5, 6, count).astype(np.float64)
+    if kind == "huge":                     # many wraps
+        return rng.uniform(-1000.0, 1000.0, count)
+    raise ValueError(kind)
+
+
+def _sweep_case(oracle, cfg, dtype, dim, kind, seed):
+    rng = np.random.default_rng(seed)
+    s = make_solver(cfg, dtype)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
+    count = cfg.N[cfg.dx + dim] if dim < cfg.dx else cfg.X
+    sigma = _random_shifts(rng, count, kind)
+    s.set_initial(f0)
+    s.translate(dim, sigma)
+    got = s.get_f()
+    ref = oracle.translate(f0.copy(), cfg.N, cfg.order, dim, sigma, dep_of(cfg.dx, dim))
+    s.close()
+    return got, ref
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("o", [1, 2, 3, 4])
+@pytest.mark.parametrize("kind", ["small", "wide", "integer", "huge"])
+def test_sweep_1p1(oracle, o, dtype, kind):
+    cfg = W.Config("t11", 1, 1, (37, 29), o, (0.0, -3.0), (5.0, 3.0))
+    for dim in (0, 1):
+        got, ref = _sweep_case(oracle, cfg, dtype, dim, kind, 10 * o + dim)
+        if kind == "integer":
+            assert np.array_equal(got, ref)
+        assert rel_err(got, ref) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("o", [2, 3])
+def test_sweep_2p2_every_direction(oracle, o, dtype):
+    cfg = W.Config("t22", 2, 2, (12, 7, 9, 10), o, (0.0,) * 4, (12.0, 7.0, 9.0, 10.0))
+    for dim in range(4):
+        for kind in ("small", "wide"):
+            got, ref = _sweep_case(oracle, cfg, dtype, dim, kind, 100 + dim)
+            assert rel_err(got, ref) <= TOL[dtype], (dim, kind)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("o", [2, 3])
+def test_sweep_3p3_every_direction(oracle, o, dtype):
+    cfg = W.Config("t33", 3, 3, (5, 4, 3, 6, 3, 4), o, (0.0,) * 6, (5.0, 4.0, 3.0, 6.0, 3.0, 4.0))
+    for dim in range(6):
+        got, ref = _sweep_case(oracle, cfg, dtype, dim, "wide", 200 + dim)
+        assert rel_err(got, ref) <= TOL[dtype], dim
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config4_reduced_twin_all_sweeps(oracle, dtype):
+    """Config 4 recipe (uniform f from the counter generator, per-cell shifts) with every n_d
+    divided by 8, 3 sweeps per direction, full element-wise parity."""
+    cfg = W.CONFIG4.scaled((16, 16, 8, 8))
+    s = make_solver(cfg, dtype)
+    s.fill_uniform(W.SEED, W.TAG_F)
+    f_host = W.uniform(W.SEED, W.TAG_F, np.arange(cfg.ndof, dtype=np.uint64)).astype(NPDT[dtype])
+    assert np.array_equal(s.get_f(), f_host)        # device generator == host generator, bit for bit
+    ref = f_host.copy()
+    for dim in range(4):
+        sigma = W.config4_shifts(cfg, dim)
+        for _ in range(3):
+            s.translate(dim, sigma)
+            oracle.translate(ref, cfg.N, cfg.order, dim, sigma, dep_of(cfg.dx, dim))
+        assert rel_err(s.get_f(), ref) <= TOL[dtype], dim
+    s.close()
+
+
+def test_long_line_and_segments(oracle):
+    """1+1 D with few long lines: the strided kernel splits lines into segments."""
+    cfg = W.Config("long", 1, 1, (6, 300), 3, (0.0, -1.0), (1.0, 1.0))
+    for kind in ("small", "wide", "huge"):
+        got, ref = _sweep_case(oracle, cfg, "f64", 1, kind, 7)
+        assert rel_err(got, ref) <= TOL["f64"], kind
+    cfg = W.Config("long2", 2, 2, (4, 150, 3, 2), 2, (0.0,) * 4, (1.0,) * 4)
+    got, ref = _sweep_case(oracle, cfg, "f64", 1, "wide", 8)
+    assert rel_err(got, ref) <= TOL["f64"]
+
+
+def test_single_cell_dimension(oracle):
+    """Degenerate: one cell along the swept dimension (i* and i*+1 are the same cell)."""
+    cfg = W.Config("one", 1, 1, (1, 5), 3, (0.0, -1.0), (1.0, 1.0))
+    got, ref = _sweep_case(oracle, cfg, "f64", 0, "wide", 3)
+    assert rel_err(got, ref) <= TOL["f64"]
+    cfg = W.Config("one", 1, 1, (5, 1), 2, (0.0, -1.0), (1.0, 1.0))
+    got, ref = _sweep_case(oracle, cfg, "f64", 1, "wide", 4)
+    assert rel_err(got, ref) <= TOL["f64"]
+
+
+def test_bad_arguments_fail_loudly():
+    from paper_1907_08316_b200.sldg import SldgError
+    cfg = W.Config("t", 1, 1, (4, 4), 2, (0.0, 0.0), (1.0, 1.0))
+    s = make_solver(cfg, "f64")
+    with pytest.raises(SldgError):
+        s.translate(0, np.zeros(3))             # wrong count
+    with pytest.raises(SldgError):
+        s.advect(1, 0.1)                        # no E stored
+    with pytest.raises(SldgError):
+        s.poisson_E()                           # no rho
+    s.close()
+    with pytest.raises(SldgError):
+        make_solver(W.Config("t", 1, 1, (4, 4), 7, (0.0, 0.0), (1.0, 1.0)), "f64")
