@@ -31,37 +31,58 @@ int oracle_num_threads(void) {
 
 /* ---- O1: Gauss-Legendre nodes/weights on [0,1] ------------------------------ */
 
-/* Legendre P_o(r) and P_o'(r) by the three-term recurrence. */
-static void legendre_pd(int o, double r, double *P, double *dP) {
-    double p0 = 1.0, p1 = r;
-    if (o == 0) { *P = 1.0; *dP = 0.0; return; }
+/* Legendre P_o(r) and P_o'(r) by the three-term recurrence.
+ *
+ * Precision note (D:O7 / D:R9 "A,B ... rounded once to T"): the nodes, the weights and the
+ * matrices A,B are DEFINED as exact real numbers (roots of P_o, exact integrals) that are
+ * rounded once.  To make "rounded once" true in practice the rule and the A,B quadrature
+ * are carried out in long double (64-bit mantissa on x86) and rounded to double at the
+ * end; a plain-double evaluation is off by up to 2 ulp in most entries, which an unstable
+ * problem (config 2) amplifies to ~3e-12 between two honest implementations. */
+static void legendre_pd(int o, long double r, long double *P, long double *dP) {
+    long double p0 = 1.0L, p1 = r;
+    if (o == 0) { *P = 1.0L; *dP = 0.0L; return; }
     for (int k = 2; k <= o; ++k) {
-        double p2 = ((2.0 * k - 1.0) * r * p1 - (k - 1.0) * p0) / k;
+        long double p2 = ((2.0L * k - 1.0L) * r * p1 - (k - 1.0L) * p0) / k;
         p0 = p1; p1 = p2;
     }
     *P = p1;
-    *dP = o * (r * p1 - p0) / (r * r - 1.0);
+    *dP = o * (r * p1 - p0) / (r * r - 1.0L);
 }
 
-int oracle_gauss_legendre(int o, double *xi, double *w) {
+static int gauss_legendre_ld(int o, long double *xi, long double *w) {
     if (o < 1 || o > ORACLE_MAX_ORDER || !xi || !w) return 1;
     for (int i = 0; i < o; ++i) {
         /* roots of P_o on [-1,1], descending in i; Newton from the Chebyshev guess */
-        double r = cos(ORACLE_PI * (i + 0.75) / (o + 0.5));
-        double P, dP;
+        long double r = cosl((long double)ORACLE_PI * (i + 0.75L) / (o + 0.5L));
+        long double P, dP;
         for (int it = 0; it < 100; ++it) {
             legendre_pd(o, r, &P, &dP);
-            double dr = P / dP;
+            long double dr = P / dP;
             r -= dr;
-            if (fabs(dr) < 1e-17) break;
+            if (fabsl(dr) < 1e-21L) break;
         }
         legendre_pd(o, r, &P, &dP);
-        double W = 2.0 / ((1.0 - r * r) * dP * dP);
-        xi[o - 1 - i] = 0.5 * (1.0 + r);   /* ascending on [0,1] */
-        w[o - 1 - i] = 0.5 * W;
+        long double W = 2.0L / ((1.0L - r * r) * dP * dP);
+        xi[o - 1 - i] = 0.5L * (1.0L + r);   /* ascending on [0,1] */
+        w[o - 1 - i] = 0.5L * W;
     }
-    if (o % 2 == 1) xi[o / 2] = 0.5;        /* the middle root is exactly r = 0 */
+    if (o % 2 == 1) xi[o / 2] = 0.5L;        /* the middle root is exactly r = 0 */
     return 0;
+}
+
+int oracle_gauss_legendre(int o, double *xi, double *w) {
+    long double xl[ORACLE_MAX_ORDER], wl[ORACLE_MAX_ORDER];
+    if (!xi || !w || gauss_legendre_ld(o, xl, wl)) return 1;
+    for (int j = 0; j < o; ++j) { xi[j] = (double)xl[j]; w[j] = (double)wl[j]; }
+    return 0;
+}
+
+static long double lagrange_ld(int o, const long double *xi, int j, long double x) {
+    long double v = 1.0L;
+    for (int m = 0; m < o; ++m)
+        if (m != j) v *= (x - xi[m]) / (xi[j] - xi[m]);
+    return v;
 }
 
 double oracle_lagrange(int o, const double *xi, int j, double x) {
@@ -92,23 +113,24 @@ void oracle_shift_split(double sigma, long *m, double *theta) {
 
 /* ---- O2: A(theta), B(theta) --------------------------------------------- */
 
-int oracle_assemble_AB(int o, double theta, double *A, double *B) {
-    double xi[ORACLE_MAX_ORDER], w[ORACLE_MAX_ORDER];
-    if (!A || !B || !(theta >= 0.0 && theta < 1.0)) return 1;
-    if (oracle_gauss_legendre(o, xi, w)) return 1;
-    double la = 1.0 - theta;   /* length of [0, 1-theta]  */
-    double lb = theta;         /* length of [1-theta, 1]  */
+int oracle_assemble_AB(int o, double theta_in, double *A, double *B) {
+    long double xi[ORACLE_MAX_ORDER], w[ORACLE_MAX_ORDER];
+    if (!A || !B || !(theta_in >= 0.0 && theta_in < 1.0)) return 1;
+    if (gauss_legendre_ld(o, xi, w)) return 1;
+    long double theta = (long double)theta_in;
+    long double la = 1.0L - theta;   /* length of [0, 1-theta]  */
+    long double lb = theta;          /* length of [1-theta, 1]  */
     for (int j = 0; j < o; ++j) {
         for (int l = 0; l < o; ++l) {
-            double sa = 0.0, sb = 0.0;
+            long double sa = 0.0L, sb = 0.0L;
             for (int q = 0; q < o; ++q) {
-                double xa = la * xi[q];            /* quadrature point in [0, 1-theta] */
-                sa += la * w[q] * oracle_lagrange(o, xi, j, xa) * oracle_lagrange(o, xi, l, xa + theta);
-                double xb = la + lb * xi[q];       /* quadrature point in [1-theta, 1] */
-                sb += lb * w[q] * oracle_lagrange(o, xi, j, xb) * oracle_lagrange(o, xi, l, lb * xi[q]);
+                long double xa = la * xi[q];            /* quadrature point in [0, 1-theta] */
+                sa += la * w[q] * lagrange_ld(o, xi, j, xa) * lagrange_ld(o, xi, l, xa + theta);
+                long double xb = la + lb * xi[q];       /* quadrature point in [1-theta, 1] */
+                sb += lb * w[q] * lagrange_ld(o, xi, j, xb) * lagrange_ld(o, xi, l, lb * xi[q]);
             }
-            A[j * o + l] = sa / w[j];
-            B[j * o + l] = sb / w[j];
+            A[j * o + l] = (double)(sa / w[j]);         /* rounded once */
+            B[j * o + l] = (double)(sb / w[j]);
         }
     }
     return 0;

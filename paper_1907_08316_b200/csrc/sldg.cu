@@ -358,7 +358,7 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
     // a-1
     {
         int block = 128;
-        size_t sh = (size_t)2 * O * O * 2 * O * sizeof(double);
+        size_t sh = (size_t)2 * O * O * 2 * O * 2 * sizeof(double);
         assemble_ab_kernel<T><<<(unsigned)cdiv(count, block), block, sh, c->stream>>>(
             c->d_sigma, count, O, n, c->d_coef, c->d_m, (T *)c->d_ab);
         LAUNCH_CHECK(c);

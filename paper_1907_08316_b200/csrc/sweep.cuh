@@ -19,19 +19,35 @@ namespace sldg {
 //     mtab[q]            = m mod n  in [0, n)
 //     ab[e*count + q]    = e-th entry of [A row-major | B row-major], e in [0, 2 o^2)
 // ------------------------------------------------------------------------------------------
+// Double-double Horner step: (hi,lo) <- (hi,lo)*theta + (chi,clo), error-free transformations
+// (two-product by FMA, two-sum by Knuth); keeps the evaluated polynomial good to ~1e-30 so the
+// single rounding to T below is the only one (D:O7 "rounded once").
+__device__ __forceinline__ void dd_horner_step(double &hi, double &lo, double theta, double chi,
+                                               double clo) {
+    double p = __dmul_rn(hi, theta);
+    double pe = __fma_rn(hi, theta, -p);           // hi*theta = p + pe exactly
+    pe = __fma_rn(lo, theta, pe);
+    double s = __dadd_rn(p, chi);                  // two-sum(p, chi)
+    double bb = __dadd_rn(s, -p);
+    double se = __dadd_rn(__dadd_rn(p, -__dadd_rn(s, -bb)), __dadd_rn(chi, -bb));
+    se = __dadd_rn(se, __dadd_rn(pe, clo));
+    hi = __dadd_rn(s, se);                         // fast two-sum renormalisation
+    lo = __dadd_rn(se, -__dadd_rn(hi, -s));
+}
+
 template <typename T>
 __global__ void assemble_ab_kernel(const double *__restrict__ sigma, long count, int o, int n,
                                    const double *__restrict__ coef, int *__restrict__ mtab,
                                    T *__restrict__ ab) {
-    extern __shared__ double s_coef[];
+    extern __shared__ double s_coef[];             // [2 o^2][2o][hi,lo]
     const int nc = 2 * o, ne = 2 * o * o;
-    for (int t = threadIdx.x; t < ne * nc; t += blockDim.x) s_coef[t] = coef[t];
+    for (int t = threadIdx.x; t < ne * nc * 2; t += blockDim.x) s_coef[t] = coef[t];
     __syncthreads();
     long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= count) return;
     double delta = -sigma[q];
     double fl = floor(delta);
-    double theta = delta - fl;
+    double theta = delta - fl;                     // exact (Sterbenz / same binade)
     // m mod n without overflow for large |shift|: fmod on the (integer-valued) double
     double mm = fmod(fl, (double)n);
     if (mm < 0.0) mm += (double)n;
@@ -39,10 +55,10 @@ __global__ void assemble_ab_kernel(const double *__restrict__ sigma, long count,
     if (m >= n) m = 0;
     mtab[q] = m;
     for (int e = 0; e < ne; ++e) {
-        const double *c = s_coef + e * nc;
-        double acc = c[nc - 1];
-        for (int k = nc - 2; k >= 0; --k) acc = fma(acc, theta, c[k]);
-        ab[(long)e * count + q] = (T)acc;
+        const double *c = s_coef + (size_t)e * nc * 2;
+        double hi = c[(nc - 1) * 2], lo = c[(nc - 1) * 2 + 1];
+        for (int k = nc - 2; k >= 0; --k) dd_horner_step(hi, lo, theta, c[k * 2], c[k * 2 + 1]);
+        ab[(long)e * count + q] = (T)hi;
     }
 }
 

@@ -104,7 +104,9 @@ inline long double binom(int n, int k) {
     return v;
 }
 
-// coef[((mat*o + j)*o + l)*(2o) + k] = coefficient of th^k in A_jl (mat=0) / B_jl (mat=1).
+// coef[(((mat*o + j)*o + l)*(2o) + k)*2 + {0,1}] = (hi, lo) double-double pair of the
+// coefficient of th^k in A_jl (mat=0) / B_jl (mat=1): hi + lo carries the long-double value,
+// so that the device's double-double Horner gives A,B that are "rounded once" (D:O7).
 inline std::vector<double> ab_polynomial_coefficients(int o) {
     long double xi[kMaxOrder], w[kMaxOrder];
     gauss_legendre_01_ld(o, xi, w);
@@ -127,7 +129,12 @@ inline std::vector<double> ab_polynomial_coefficients(int o) {
         for (int k = 0; k < o; ++k) c[j][k] = p[k];
     }
     const int nc = 2 * o;
-    std::vector<double> coef((size_t)2 * o * o * nc, 0.0);
+    std::vector<double> coef((size_t)2 * o * o * nc * 2, 0.0);
+    auto put = [&](size_t idx, long double v) {
+        double hi = (double)v;
+        coef[idx * 2] = hi;
+        coef[idx * 2 + 1] = (double)(v - (long double)hi);
+    };
     for (int j = 0; j < o; ++j)
         for (int l = 0; l < o; ++l) {
             PolyLD PA, PB;
@@ -146,13 +153,13 @@ inline std::vector<double> ab_polynomial_coefficients(int o) {
                     }
                 }
             for (int k = 0; k < nc; ++k) {
-                coef[((size_t)(0 * o + j) * o + l) * nc + k] = (double)(PA.c[k] / w[j]);
-                coef[((size_t)(1 * o + j) * o + l) * nc + k] = (double)(PB.c[k] / w[j]);
+                put(((size_t)(0 * o + j) * o + l) * nc + k, PA.c[k] / w[j]);
+                put(((size_t)(1 * o + j) * o + l) * nc + k, PB.c[k] / w[j]);
             }
             // theta = 0: A = I and B = 0 exactly (int_0^1 l_j l_l = w_j delta_jl because the o-point
             // rule is exact for degree 2o-2), so integer shifts move data bit-exactly (D:R3, P4).
-            coef[((size_t)(0 * o + j) * o + l) * nc] = (j == l) ? 1.0 : 0.0;
-            coef[((size_t)(1 * o + j) * o + l) * nc] = 0.0;
+            put(((size_t)(0 * o + j) * o + l) * nc, (j == l) ? 1.0L : 0.0L);
+            put(((size_t)(1 * o + j) * o + l) * nc, 0.0L);
         }
     return coef;
 }
