@@ -9,8 +9,6 @@ import os
 
 import numpy as np
 
-from . import build as _build
-
 SLDG_F64, SLDG_F32 = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -163,12 +161,19 @@ class Sldg:
     def advect(self, dim, dt):
         self._chk(_lib.sldg_advect(self.h, dim, float(dt)), "advect")
 
-    def compute_rho(self):
+    def compute_rho(self, out=True):
+        """rho into the context; with out=True also returned as a new device tensor."""
+        if not out:
+            self._chk(_lib.sldg_compute_rho(self.h, None), "compute_rho")
+            return None
         rho = self.torch.empty(self.X, dtype=self.torch.float64, device=self.device)
         self._chk(_lib.sldg_compute_rho(self.h, rho.data_ptr()), "compute_rho")
         return rho
 
-    def poisson_E(self):
+    def poisson_E(self, out=True):
+        if not out:
+            self._chk(_lib.sldg_poisson_E(self.h, None), "poisson_E")
+            return None
         E = self.torch.empty((self.dx, self.X), dtype=self.torch.float64, device=self.device)
         self._chk(_lib.sldg_poisson_E(self.h, E.data_ptr()), "poisson_E")
         return E
