@@ -7,6 +7,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -15,6 +16,7 @@
 #include "poisson.cuh"
 #include "reduce.cuh"
 #include "sweep.cuh"
+#include "sweep_tma.cuh"
 #include "tables.hpp"
 
 using namespace sldg;
@@ -55,6 +57,7 @@ struct sldg_ctx {
     double *d_t[4] = {nullptr, nullptr, nullptr, nullptr};   // complex scratch (re, im) x 2
     double *d_gh[2] = {nullptr, nullptr};                    // g_hat (re, im) [KK]
 
+    bool use_tma = true;               // SLDG_NO_TMA=1 in the environment selects the plain kernels
     bool have_rho = false, have_E = false;
     unsigned long long launches = 0;
     char err[512] = "";
@@ -168,6 +171,10 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         if (d < dx) c->X *= c->N[d]; else c->V *= c->N[d];
     }
     gauss_legendre_01(order, c->xi, c->w);
+    {
+        const char *e = getenv("SLDG_NO_TMA");
+        c->use_tma = !(e && e[0] == '1');
+    }
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -372,12 +379,36 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
         for (int d = 1; d < c->dx; ++d) qdiv *= c->N[d];
         long ngroups = outer / qdiv;
         long cpg = qdiv * n;                       // cells per group
-        int block = 256;
-        int cpb = 2048;                            // cells per block
-        if (cpg < cpb) { cpb = (int)cpg; if (cpb < block) block = (int)(cdiv(cpb, 32) * 32); }
-        int bpg = (int)cdiv(cpg, cpb);
-        sweep_x1_kernel<T, O><<<(unsigned)(ngroups * bpg), block, 0, c->stream>>>(
-            in, out, n, ngroups, cpg, cpb, bpg, c->d_m, (const T *)c->d_ab, count, c->N[c->dx]);
+        const size_t line_bytes = (size_t)n * O * sizeof(T);
+        bool done = false;
+        if (c->use_tma && line_bytes % 16 == 0 && line_bytes <= 96 * 1024) {
+            // staged variant: R whole lines per block through shared memory (bulk copies)
+            long R = (32 * 1024) / (long)line_bytes;
+            if (R < 1) R = 1;
+            if (R > qdiv) R = qdiv;
+            int chunks = (int)cdiv(qdiv, R);
+            size_t half = ((size_t)R * line_bytes + 127) & ~(size_t)127;
+            size_t smem = 2 * half;
+            static size_t attr_set = 0;
+            if (smem > attr_set) {
+                cudaFuncSetAttribute(sweep_x1_bulk_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+                attr_set = 200 * 1024;
+            }
+            long ncell = R * n;
+            int block = ncell >= 256 ? 256 : (int)(cdiv(ncell, 32) * 32);
+            if (block < 64) block = 64;
+            sweep_x1_bulk_kernel<T, O><<<(unsigned)(ngroups * chunks), block, smem, c->stream>>>(
+                in, out, n, qdiv, (int)R, chunks, c->d_m, (const T *)c->d_ab, count, c->N[c->dx]);
+            done = true;
+        }
+        if (!done) {
+            int block = 256;
+            int cpb = 2048;                        // cells per block
+            if (cpg < cpb) { cpb = (int)cpg; if (cpb < block) block = (int)(cdiv(cpb, 32) * 32); }
+            int bpg = (int)cdiv(cpg, cpb);
+            sweep_x1_kernel<T, O><<<(unsigned)(ngroups * bpg), block, 0, c->stream>>>(
+                in, out, n, ngroups, cpg, cpb, bpg, c->d_m, (const T *)c->d_ab, count, c->N[c->dx]);
+        }
     } else if (dim < c->dx) {
         const int dep = c->dx + dim;
         long qdiv = 1;
@@ -388,7 +419,37 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
         else if (inner % 2 == 0) launch_strided<T, O, 2, false>(c, in, out, inner, n, outer, count, qdiv, qmod);
         else launch_strided<T, O, 1, false>(c, in, out, inner, n, outer, count, qdiv, qmod);
     } else {
-        launch_strided<T, O, 1, true>(c, in, out, inner, n, outer, count, 1, 1);
+        bool done = false;
+        const long Nk = (long)n * O;
+        int W = 256 / (int)sizeof(T);
+        int nbox = (int)cdiv(Nk, 256);
+        int box_rows = (int)cdiv(Nk, nbox);
+        while (W > 8 && (size_t)nbox * box_rows * W * sizeof(T) > 100 * 1024) W /= 2;
+        {   // every TMA box must land on a 128-byte aligned shared-memory address
+            int align = 128 / (W * (int)sizeof(T));
+            if (align > 1) box_rows = (int)(cdiv(box_rows, align) * align);
+            if (box_rows > 256) { nbox += 1; box_rows = (int)(cdiv(cdiv(Nk, nbox), align > 1 ? align : 1) * (align > 1 ? align : 1)); }
+        }
+        size_t smem = (size_t)nbox * box_rows * W * sizeof(T);
+        if (c->use_tma && (inner * sizeof(T)) % 16 == 0 && inner >= W && smem <= 200 * 1024 &&
+            inner < (1L << 31) && outer < (1L << 31)) {
+            CUtensorMap tmap;
+            if (make_tensor_map_3d(&tmap, in, sizeof(T) == 8, (uint64_t)inner, (uint64_t)Nk, (uint64_t)outer,
+                                   (uint32_t)W, (uint32_t)box_rows)) {
+                static bool attr_set = false;
+                if (!attr_set) {
+                    cudaFuncSetAttribute(sweep_tile_tma_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+                    attr_set = true;
+                }
+                int nseg = 128 / W;
+                int cps = (int)cdiv(n, nseg);
+                long tpo = cdiv(inner, W);
+                sweep_tile_tma_kernel<T, O><<<(unsigned)(tpo * outer), 128, smem, c->stream>>>(
+                    tmap, out, inner, n, tpo, W, nbox, box_rows, cps, c->d_m, (const T *)c->d_ab, count, c->X);
+                done = true;
+            }
+        }
+        if (!done) launch_strided<T, O, 1, true>(c, in, out, inner, n, outer, count, 1, 1);
     }
     LAUNCH_CHECK(c);
     c->cur ^= 1;

@@ -1,0 +1,171 @@
+// sweep_tma.cuh -- the sm_100a staged variants of the translation sweep (row a-2):
+// whole lines are brought into shared memory by the asynchronous copy engine (TMA), so that
+//   * every byte of f is read from HBM exactly once and in full, aligned rows, whatever the
+//     per-line cell offset m is (the config-4 shifts scatter m over 8 values inside a warp);
+//   * the load/store units only see conflict-free shared-memory reads and coalesced stores.
+// Same arithmetic contract as sweep.cuh (D:O7).
+#pragma once
+#include "sweep.cuh"
+#include "tma.cuh"
+
+namespace sldg {
+
+// ------------------------------------------------------------------------------------------
+// v_a sweeps (and any sweep whose shift varies along `inner`): f viewed as
+// [outer][N_k][inner]; one block owns the tile [all N_k rows] x [W consecutive inner
+// indices] of one `outer` index, loaded by nbox TMA boxes of box_rows rows each.
+// Thread (col, seg): column `col` of the tile, cells [seg*cps, (seg+1)*cps); q = ii % X.
+// The line is periodic and entirely in shared memory, so m is free per thread.
+// Outputs go straight from registers to global (row-contiguous across the warp).
+// ------------------------------------------------------------------------------------------
+template <typename T, int O>
+__global__ void __launch_bounds__(128)
+sweep_tile_tma_kernel(const __grid_constant__ CUtensorMap tmap, T *__restrict__ out, long inner, int n,
+                      long tiles_per_outer, int W, int nbox, int box_rows, int cps,
+                      const int *__restrict__ mtab, const T *__restrict__ ab, long count, long X) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t bar;
+    T *tile = reinterpret_cast<T *>(smem_raw);                  // [nbox*box_rows][W]
+    const long tile_id = blockIdx.x;
+    const long oo = tile_id / tiles_per_outer;
+    const long col0 = (tile_id - oo * tiles_per_outer) * W;
+    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        mbar_expect_tx(&bar, (uint32_t)((size_t)nbox * box_rows * W * sizeof(T)));
+        for (int b = 0; b < nbox; ++b)
+            tma_load_3d(tile + (size_t)b * box_rows * W, &tmap, (int)col0, b * box_rows, (int)oo, &bar);
+    }
+    const int col = threadIdx.x % W;
+    const int seg = threadIdx.x / W;
+    const long ii = col0 + col;
+    const bool valid = ii < inner;
+    const long q = valid ? (ii % X) : 0;
+    T A[O * O], B[O * O];
+#pragma unroll
+    for (int e = 0; e < O * O; ++e) {
+        A[e] = ab[(long)e * count + q];
+        B[e] = ab[(long)(O * O + e) * count + q];
+    }
+    const int m = mtab[q];
+    mbar_wait(&bar, 0);
+    const int c0 = seg * cps;
+    int c1 = c0 + cps;
+    if (c1 > n) c1 = n;
+    if (!valid || c0 >= c1) return;
+
+    const T *colp = tile + col;
+    int is = c0 + m;
+    if (is >= n) is -= n;
+    T u0[O], u1[O];
+#pragma unroll
+    for (int l = 0; l < O; ++l) u0[l] = colp[(is * O + l) * W];
+    T *dst = out + (oo * (long)n * O + (long)c0 * O) * inner + ii;
+#pragma unroll 2
+    for (int c = c0; c < c1; ++c) {
+        if (++is == n) is = 0;
+#pragma unroll
+        for (int l = 0; l < O; ++l) u1[l] = colp[(is * O + l) * W];
+#pragma unroll
+        for (int j = 0; j < O; ++j) dst[(long)j * inner] = chain<T, O>(A, B, j, u0, u1);
+#pragma unroll
+        for (int l = 0; l < O; ++l) u0[l] = u1[l];
+        dst += (long)O * inner;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// x_1 sweep (contiguous lines): a block owns R whole consecutive lines of one shift group
+// (one contiguous span of global memory): one bulk copy in, thread-per-cell arithmetic from
+// shared to shared, one bulk copy out.  Cell reads have a stride of O words (conflict-free
+// for O = 1..4 with 8- and 4-byte words except O = 4, which is 2-way), and the copy engine
+// does all global traffic in full 128-byte lines.
+// ------------------------------------------------------------------------------------------
+template <typename T, int O>
+__device__ __forceinline__ void load_cell(const T *p, T (&u)[O]) {
+    if constexpr (O % 2 == 0) {
+        using V2 = Vec<T, 2>;
+#pragma unroll
+        for (int l = 0; l < O; l += 2) {
+            V2 t = *reinterpret_cast<const V2 *>(p + l);
+            u[l] = t.v[0]; u[l + 1] = t.v[1];
+        }
+    } else {
+#pragma unroll
+        for (int l = 0; l < O; ++l) u[l] = p[l];
+    }
+}
+
+template <typename T, int O>
+__global__ void __launch_bounds__(256)
+sweep_x1_bulk_kernel(const T *__restrict__ in, T *__restrict__ out, int n, long lines_per_group, int R,
+                     int chunks_per_group, const int *__restrict__ mtab, const T *__restrict__ ab,
+                     long count, long qmod) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t bar;
+    __shared__ T s_ab[2 * O * O];
+    __shared__ int s_m;
+    const long g = blockIdx.x / chunks_per_group;
+    const int ch = blockIdx.x - (int)(g * chunks_per_group);
+    const long line0 = (long)ch * R;
+    int nl = R;
+    if (line0 + nl > lines_per_group) nl = (int)(lines_per_group - line0);
+    const int ncell = nl * n;
+    const uint32_t bytes = (uint32_t)((size_t)ncell * O * sizeof(T));
+    const size_t half = ((size_t)R * n * O * sizeof(T) + 127) & ~(size_t)127;
+    T *s_in = reinterpret_cast<T *>(smem_raw);
+    T *s_out = reinterpret_cast<T *>(smem_raw + half);
+    const long base = (g * lines_per_group + line0) * (long)n * O;
+
+    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        mbar_expect_tx(&bar, bytes);
+        bulk_g2s(s_in, in + base, bytes, &bar);
+    }
+    const long q = g % qmod;
+    if (threadIdx.x < 2 * O * O) s_ab[threadIdx.x] = ab[(long)threadIdx.x * count + q];
+    if (threadIdx.x == 32) s_m = mtab[q];
+    __syncthreads();
+    T A[O * O], B[O * O];
+#pragma unroll
+    for (int e = 0; e < O * O; ++e) { A[e] = s_ab[e]; B[e] = s_ab[O * O + e]; }
+    const int m = s_m;
+    mbar_wait(&bar, 0);
+
+    for (int c = threadIdx.x; c < ncell; c += blockDim.x) {
+        const int line = c / n;
+        const int i = c - line * n;
+        int is = i + m;
+        if (is >= n) is -= n;
+        int is1 = is + 1;
+        if (is1 == n) is1 = 0;
+        T u0[O], u1[O];
+        load_cell<T, O>(s_in + (size_t)(line * n + is) * O, u0);
+        load_cell<T, O>(s_in + (size_t)(line * n + is1) * O, u1);
+        T r[O];
+#pragma unroll
+        for (int j = 0; j < O; ++j) r[j] = chain<T, O>(A, B, j, u0, u1);
+        T *po = s_out + (size_t)c * O;
+        if constexpr (O % 2 == 0) {
+            using V2 = Vec<T, 2>;
+#pragma unroll
+            for (int j = 0; j < O; j += 2) {
+                V2 t; t.v[0] = r[j]; t.v[1] = r[j + 1];
+                *reinterpret_cast<V2 *>(po + j) = t;
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < O; ++j) po[j] = r[j];
+        }
+    }
+    fence_proxy_async();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        bulk_s2g(out + base, s_out, bytes);
+        bulk_commit();
+        bulk_wait_read0();
+    }
+}
+
+}  // namespace sldg
