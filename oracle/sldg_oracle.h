@@ -15,7 +15,8 @@
  * local Gauss-Legendre node j); f is a dense array with linear index
  * sum_d p_d * prod_{e<d} N_e (x_1 fastest).  All directions are periodic (R5).
  * Everything is fp64 except f itself and the rounded A,B in the *_f32 variants
- * (R9).  Every function returns 0 on success, nonzero on a bad argument.
+ * (R9); the Gauss-Legendre rule and the A,B quadrature are carried out in long double
+ * internally and rounded ONCE to double (O7: 'rounded once' taken literally).  Every function returns 0 on success, nonzero on a bad argument.
  *
  * Pins (tests/test_oracle_pins.py): P1..P13 of S:§8(c).  Config-2 two-stream
  * growth is "parity unpinned" by the paper (its eq. (2) is a different state).
