@@ -238,6 +238,22 @@ def sweep_table(torch, s, cfg, dtype, reps, warm):
     return out
 
 
+def max_over_ranks(values, world, device):
+    """Element-wise MAX of a list of floats over all ranks (timings are max-over-ranks)."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def replica_throughput(world, bytes_per_replica, ms_max):
+    """Whole-job GB/s of `world` independent replicas that each moved bytes_per_replica in ms_max."""
+    return world * bytes_per_replica / ms_max / 1e6
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -307,12 +323,9 @@ def run_ours(args):
         per_dim[d].append(e0.elapsed_time(e1))
     sweep_ms = sum(sum(v) for v in per_dim.values())
     nsweeps = sum(len(v) for v in per_dim.values())
-    if world > 1:
-        tt = torch.tensor([total_ms, sweep_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms, sweep_ms = float(tt[0]), float(tt[1])
+    total_ms, sweep_ms = max_over_ranks([total_ms, sweep_ms], world, "cuda")
     sweep_bytes = 2.0 * cfg.ndof * es
-    value = world * sweep_bytes * nsweeps / sweep_ms / 1e6               # GB/s per sweep, all replicas
+    value = replica_throughput(world, sweep_bytes * nsweeps, sweep_ms)   # GB/s per sweep, all replicas
     # dominant kernel = slowest direction's sweep kernel
     dim_avg = {d: float(np.mean(v)) for d, v in per_dim.items()}
     dom = max(dim_avg, key=dim_avg.get)
@@ -357,10 +370,7 @@ def run_ours(args):
                 s.get_f(hbuf)
             torch.cuda.synchronize()
             dt = time.perf_counter() - t0
-            if world > 1:
-                tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
-                dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-                dt = float(tt[0])
+            dt = max_over_ranks([dt], world, "cuda")[0]
             line["e2e"] = {"value": world * sweep_bytes * D * k / dt / 1e9, "unit": UNIT,
                            "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 24,
                            "ms_per_step": 1e3 * dt / k, "steps": k, "note": e2e_note +

@@ -1,0 +1,63 @@
+"""CPU, world_size 2, gloo: the N > 1 host logic of bench.py ("replicas only"):
+timings are reduced with MAX over ranks, the whole-job value is the sum over replicas, and only
+rank 0 of the reference arm does work."""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, out):
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%d" % port, rank=rank, world_size=world)
+    # rank r pretends its timed region took (10 + 5 r) ms in total and (8 + r) ms in the sweeps
+    total, sweeps = bench.max_over_ranks([10.0 + 5.0 * rank, 8.0 + rank], world, "cpu")
+    val = bench.replica_throughput(world, 1e9, sweeps)
+    dist.barrier()
+    if rank == 0:
+        out.put((total, sweeps, val))
+    dist.destroy_process_group()
+
+
+def test_max_over_ranks_and_replica_sum_world2():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    total, sweeps, val = q.get(timeout=120)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert total == 15.0 and sweeps == 9.0            # MAX over ranks, not rank 0's own 10 / 8
+    assert abs(val - 2 * 1e9 / 9.0 / 1e6) < 1e-9       # two replicas' bytes over the slowest rank's time
+
+
+def test_single_rank_is_identity():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.max_over_ranks([3.0, 4.0], 1, "cpu") == [3.0, 4.0]
+    assert bench.replica_throughput(1, 2e9, 1.0) == 2000.0
+
+
+def test_reference_arm_only_rank0_prints():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0 and r.stdout.strip() == ""

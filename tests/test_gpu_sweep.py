@@ -119,3 +119,33 @@ def test_bad_arguments_fail_loudly():
     s.close()
     with pytest.raises(SldgError):
         make_solver(W.Config("t", 1, 1, (4, 4), 7, (0.0, 0.0), (1.0, 1.0)), "f64")
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_plain_kernels_without_tma(oracle, dtype, monkeypatch):
+    """SLDG_NO_TMA=1 selects the register-window / thread-per-cell kernels that also serve as
+    fallbacks when the TMA preconditions fail; they must give the same results."""
+    monkeypatch.setenv("SLDG_NO_TMA", "1")
+    cfg = W.Config("t22", 2, 2, (12, 8, 9, 10), 3, (0.0,) * 4, (12.0, 8.0, 9.0, 10.0))
+    for dim in range(4):
+        got, ref = _sweep_case(oracle, cfg, dtype, dim, "wide", 300 + dim)
+        assert rel_err(got, ref) <= TOL[dtype], dim
+    cfg = W.Config("t11", 1, 1, (37, 29), 2, (0.0, -3.0), (5.0, 3.0))
+    for dim in (0, 1):
+        got, ref = _sweep_case(oracle, cfg, dtype, dim, "huge", 310 + dim)
+        assert rel_err(got, ref) <= TOL[dtype], dim
+
+
+def test_tma_and_plain_kernels_agree_bit_for_bit(monkeypatch):
+    """Same FMA chains on both routes (D:O7): identical bits, at a size spanning many tiles."""
+    cfg = W.CONFIG4.scaled((32, 16, 8, 8))
+    outs = []
+    for flag in ("0", "1"):
+        monkeypatch.setenv("SLDG_NO_TMA", flag)
+        s = make_solver(cfg, "f64")
+        s.fill_uniform(W.SEED, W.TAG_F)
+        for dim in range(4):
+            s.translate(dim, W.config4_shifts(cfg, dim))
+        outs.append(s.get_f())
+        s.close()
+    assert np.array_equal(outs[0], outs[1])
