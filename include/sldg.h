@@ -105,6 +105,15 @@ int sldg_translate_dev(sldg_ctx *ctx, int dim, const double *shift_cells_device,
  * dim >= dx: sigma = -E_a(x_q) dt / h_{v_a} with the stored E (SLDG_ERR_STATE if none). */
 int sldg_advect(sldg_ctx *ctx, int dim, double dt);
 
+/* Two consecutive sweeps in ONE pass over f: the result is identical, bit for
+ * bit, to sldg_advect(dim1, dt) followed by sldg_advect(dim2, dt) (resp. two sldg_translate_dev
+ * calls), but f is read and written once instead of twice.  dim1 < dim2, both x-dimensions or both
+ * v-dimensions (their shifts do not depend on each other's coordinate, D:R8).  sldg_step uses this
+ * for (x_1,x_2) and (v_1,v_2) unless SLDG_NO_FUSE=1 is set in the environment at sldg_create. */
+int sldg_advect_pair(sldg_ctx *ctx, int dim1, int dim2, double dt);
+int sldg_translate_pair_dev(sldg_ctx *ctx, int dim1, const double *shift1_device, size_t count1,
+                            int dim2, const double *shift2_device, size_t count2);
+
 /* rho[X] = -sum_v W_v f[v][x] (fp64 accumulation for both dtypes) into the
  * context and, if rho_device_or_null != NULL, also to that device array. */
 int sldg_compute_rho(sldg_ctx *ctx, double *rho_device_or_null);

@@ -17,6 +17,7 @@
 #include "reduce.cuh"
 #include "sweep.cuh"
 #include "sweep_tma.cuh"
+#include "sweep_fused.cuh"
 #include "tables.hpp"
 
 using namespace sldg;
@@ -46,6 +47,9 @@ struct sldg_ctx {
     double *d_sigma = nullptr;         // [tab_cap]
     int *d_m = nullptr;                // [tab_cap]
     void *d_ab = nullptr;              // [2 o^2][tab_cap] of T
+    double *d_sigma2 = nullptr;        // second table set (second sweep of a fused pair)
+    int *d_m2 = nullptr;
+    void *d_ab2 = nullptr;
     double *d_Wv = nullptr, *d_Wx = nullptr;      // quadrature weights over v-nodes / x-nodes
     double *d_rho = nullptr, *d_s2 = nullptr, *d_E = nullptr;   // [X], [X], [dx][X]
     int max_splits = 1;
@@ -57,6 +61,7 @@ struct sldg_ctx {
     double *d_t[4] = {nullptr, nullptr, nullptr, nullptr};   // complex scratch (re, im) x 2
     double *d_gh[2] = {nullptr, nullptr};                    // g_hat (re, im) [KK]
 
+    bool use_fuse = true;              // SLDG_NO_FUSE=1: sldg_step issues one sweep per pass
     bool use_tma = true;               // SLDG_NO_TMA=1 in the environment selects the plain kernels
     bool have_rho = false, have_E = false;
     unsigned long long launches = 0;
@@ -102,6 +107,7 @@ void free_tables(sldg_ctx *c) {
     cudaFree(c->d_coef);
     for (int d = 0; d < SLDG_MAX_DIM; ++d) cudaFree(c->d_coords[d]);
     cudaFree(c->d_sigma); cudaFree(c->d_m); cudaFree(c->d_ab);
+    cudaFree(c->d_sigma2); cudaFree(c->d_m2); cudaFree(c->d_ab2);
     cudaFree(c->d_Wv); cudaFree(c->d_Wx);
     cudaFree(c->d_rho); cudaFree(c->d_s2); cudaFree(c->d_E);
     cudaFree(c->d_part); cudaFree(c->d_scal);
@@ -174,6 +180,8 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
     {
         const char *e = getenv("SLDG_NO_TMA");
         c->use_tma = !(e && e[0] == '1');
+        e = getenv("SLDG_NO_FUSE");
+        c->use_fuse = !(e && e[0] == '1');
     }
     int dev = 0;
     cudaGetDevice(&dev);
@@ -206,6 +214,9 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
     CREATE_TRY(dalloc(&c->d_sigma, c->tab_cap));
     CREATE_TRY(dalloc(&c->d_m, c->tab_cap));
     CREATE_TRY(cudaMalloc(&c->d_ab, (size_t)2 * order * order * c->tab_cap * c->esize));
+    CREATE_TRY(dalloc(&c->d_sigma2, c->tab_cap));
+    CREATE_TRY(dalloc(&c->d_m2, c->tab_cap));
+    CREATE_TRY(cudaMalloc(&c->d_ab2, (size_t)2 * order * order * c->tab_cap * c->esize));
 
     // quadrature weights W_v = prod_a h_va w_ja (v_1 fastest), W_x likewise
     {
@@ -472,6 +483,67 @@ int run_sweep(sldg_ctx *c, int dim, long count) {
     return c->dtype == SLDG_F64 ? run_sweep_o<double>(c, dim, count) : run_sweep_o<float>(c, dim, count);
 }
 
+// ---- fused pair of sweeps (sweep_fused.cuh); d_sigma / d_sigma2 hold the two shift tables ----
+template <typename T, int O>
+int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
+    const int n1 = c->cells[k1], n2 = c->cells[k2];
+    const T *in = (const T *)c->buf[c->cur];
+    T *out = (T *)c->buf[c->cur ^ 1];
+    int block = 128;
+    size_t sh = (size_t)2 * O * O * 2 * O * 2 * sizeof(double);
+    assemble_ab_kernel<T><<<(unsigned)cdiv(count1, block), block, sh, c->stream>>>(
+        c->d_sigma, count1, O, n1, c->d_coef, c->d_m, (T *)c->d_ab);
+    LAUNCH_CHECK(c);
+    assemble_ab_kernel<T><<<(unsigned)cdiv(count2, block), block, sh, c->stream>>>(
+        c->d_sigma2, count2, O, n2, c->d_coef, c->d_m2, (T *)c->d_ab2);
+    LAUNCH_CHECK(c);
+    long inner1 = 1, midN = 1, outer2 = 1;
+    for (int d = 0; d < k1; ++d) inner1 *= c->N[d];
+    for (int d = k1 + 1; d < k2; ++d) midN *= c->N[d];
+    for (int d = k2 + 1; d < c->D; ++d) outer2 *= c->N[d];
+    auto qmap = [&](int k, long &qdiv, long &qmod) {
+        if (k < c->dx) {
+            qdiv = 1;
+            for (int d = 0; d < c->dx + k; ++d) qdiv *= c->N[d];
+            qmod = c->N[c->dx + k];
+        } else { qdiv = 1; qmod = c->X; }
+    };
+    long qd1, qm1, qd2, qm2;
+    qmap(k1, qd1, qm1);
+    qmap(k2, qd2, qm2);
+    long lines = inner1 * n1 * midN * outer2;
+    long target = (long)c->sm_count * 1024;
+    int nseg = 1;
+    if (lines < target) {
+        nseg = (int)cdiv(target, lines);
+        int maxseg = n2 / 4 > 0 ? n2 / 4 : 1;
+        if (nseg > maxseg) nseg = maxseg;
+    }
+    int cps = (int)cdiv(n2, nseg);
+    nseg = (int)cdiv(n2, cps);
+    long threads = lines * nseg;
+    sweep_pair_kernel<T, O><<<(unsigned)cdiv(threads, 128), 128, 0, c->stream>>>(
+        in, out, inner1, n1, midN, n2, outer2, nseg, cps, c->d_m, (const T *)c->d_ab, count1, qd1, qm1,
+        c->d_m2, (const T *)c->d_ab2, count2, qd2, qm2);
+    LAUNCH_CHECK(c);
+    c->cur ^= 1;
+    c->have_rho = false;
+    return SLDG_OK;
+}
+
+int run_pair(sldg_ctx *c, int k1, int k2, long count1, long count2) {
+#define PAIR_CASE(TT)                                                           \
+    switch (c->o) {                                                             \
+    case 1: return run_pair_t<TT, 1>(c, k1, k2, count1, count2);                \
+    case 2: return run_pair_t<TT, 2>(c, k1, k2, count1, count2);                \
+    case 3: return run_pair_t<TT, 3>(c, k1, k2, count1, count2);                \
+    case 4: return run_pair_t<TT, 4>(c, k1, k2, count1, count2);                \
+    }
+    if (c->dtype == SLDG_F64) { PAIR_CASE(double) } else { PAIR_CASE(float) }
+#undef PAIR_CASE
+    return fail(c, SLDG_ERR_UNSUPPORTED, "order %d not instantiated", c->o);
+}
+
 long sweep_count(const sldg_ctx *c, int dim) { return dim < c->dx ? c->N[c->dx + dim] : c->X; }
 
 }  // namespace
@@ -493,23 +565,59 @@ extern "C" int sldg_translate_dev(sldg_ctx *c, int dim, const double *shift, siz
     return run_sweep(c, dim, (long)count);
 }
 
-extern "C" int sldg_advect(sldg_ctx *c, int dim, double dt) {
-    if (!c || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
+namespace {
+// sigma of a physics sweep (D:O3, D:R4) into `sigma` on the stream
+int fill_physics_sigma(sldg_ctx *c, int dim, double dt, double *sigma) {
     long count = sweep_count(c, dim);
     int block = 256;
     if (dim < c->dx) {
         int va = c->dx + dim;
         sigma_from_coords_kernel<<<(unsigned)cdiv(count, block), block, 0, c->stream>>>(
-            c->d_coords[va], count, dt, c->h[dim], c->d_sigma);
+            c->d_coords[va], count, dt, c->h[dim], sigma);
     } else {
         int a = dim - c->dx;
         if (a >= c->dx) return fail(c, SLDG_ERR_ARG, "sldg_advect: v_%d has no field component (dx = %d)", a + 1, c->dx);
         if (!c->have_E) return fail(c, SLDG_ERR_STATE, "sldg_advect: no E stored (call sldg_poisson_E or sldg_set_E)");
         sigma_from_E_kernel<<<(unsigned)cdiv(count, block), block, 0, c->stream>>>(
-            c->d_E + (long)a * c->X, count, dt, c->h[dim], c->d_sigma);
+            c->d_E + (long)a * c->X, count, dt, c->h[dim], sigma);
     }
     LAUNCH_CHECK(c);
-    return run_sweep(c, dim, count);
+    return SLDG_OK;
+}
+
+bool pair_ok(const sldg_ctx *c, int d1, int d2) {
+    if (d1 < 0 || d2 <= d1 || d2 >= c->D) return false;
+    return (d2 < c->dx) || (d1 >= c->dx);          // both x-dimensions or both v-dimensions
+}
+}  // namespace
+
+extern "C" int sldg_advect(sldg_ctx *c, int dim, double dt) {
+    if (!c || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
+    int rc = fill_physics_sigma(c, dim, dt, c->d_sigma);
+    if (rc) return rc;
+    return run_sweep(c, dim, sweep_count(c, dim));
+}
+
+extern "C" int sldg_advect_pair(sldg_ctx *c, int dim1, int dim2, double dt) {
+    if (!c) return SLDG_ERR_ARG;
+    if (!pair_ok(c, dim1, dim2))
+        return fail(c, SLDG_ERR_ARG, "sldg_advect_pair: need dim1 < dim2, both x- or both v-dimensions");
+    int rc = fill_physics_sigma(c, dim1, dt, c->d_sigma);
+    if (rc) return rc;
+    if ((rc = fill_physics_sigma(c, dim2, dt, c->d_sigma2))) return rc;
+    return run_pair(c, dim1, dim2, sweep_count(c, dim1), sweep_count(c, dim2));
+}
+
+extern "C" int sldg_translate_pair_dev(sldg_ctx *c, int dim1, const double *shift1, size_t count1, int dim2,
+                                       const double *shift2, size_t count2) {
+    if (!c || !shift1 || !shift2) return SLDG_ERR_ARG;
+    if (!pair_ok(c, dim1, dim2))
+        return fail(c, SLDG_ERR_ARG, "sldg_translate_pair_dev: need dim1 < dim2, both x- or both v-dimensions");
+    if ((long)count1 != sweep_count(c, dim1) || (long)count2 != sweep_count(c, dim2))
+        return fail(c, SLDG_ERR_ARG, "sldg_translate_pair_dev: wrong shift counts");
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift1, count1 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma2, shift2, count2 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    return run_pair(c, dim1, dim2, (long)count1, (long)count2);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -643,14 +751,27 @@ extern "C" int sldg_set_E(sldg_ctx *c, const double *E, int is_device) {
     return SLDG_OK;
 }
 
+namespace {
+// sweeps along dimensions base .. base+cnt-1 with increment tau, fusing the first two when allowed
+int advect_group(sldg_ctx *c, int base, int cnt, double tau) {
+    int rc, a = 0;
+    if (c->use_fuse && cnt >= 2) {
+        if ((rc = sldg_advect_pair(c, base, base + 1, tau))) return rc;
+        a = 2;
+    }
+    for (; a < cnt; ++a) if ((rc = sldg_advect(c, base + a, tau))) return rc;
+    return SLDG_OK;
+}
+}  // namespace
+
 extern "C" int sldg_step(sldg_ctx *c, double dt) {
     if (!c) return SLDG_ERR_ARG;
     int rc;
-    for (int a = 0; a < c->dx; ++a) if ((rc = sldg_advect(c, a, 0.5 * dt))) return rc;
+    if ((rc = advect_group(c, 0, c->dx, 0.5 * dt))) return rc;
     if ((rc = run_rho(c, nullptr, false))) return rc;
     if ((rc = run_poisson(c, nullptr))) return rc;
-    for (int a = 0; a < c->dx; ++a) if ((rc = sldg_advect(c, c->dx + a, dt))) return rc;
-    for (int a = 0; a < c->dx; ++a) if ((rc = sldg_advect(c, a, 0.5 * dt))) return rc;
+    if ((rc = advect_group(c, c->dx, c->dx, dt))) return rc;
+    if ((rc = advect_group(c, 0, c->dx, 0.5 * dt))) return rc;
     return SLDG_OK;
 }
 

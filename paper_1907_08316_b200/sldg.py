@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libsldg.so")
 EXPORTS = [
     "sldg_create", "sldg_destroy", "sldg_last_error", "sldg_num_dofs", "sldg_num_x",
     "sldg_node_coords", "sldg_set_initial", "sldg_get_f", "sldg_current", "sldg_fill_uniform",
-    "sldg_translate", "sldg_translate_dev", "sldg_advect", "sldg_compute_rho", "sldg_poisson_E",
+    "sldg_translate", "sldg_translate_dev", "sldg_advect", "sldg_advect_pair", "sldg_translate_pair_dev", "sldg_compute_rho", "sldg_poisson_E",
     "sldg_set_E", "sldg_step", "sldg_diagnostics", "sldg_launch_count",
 ]
 
@@ -46,6 +46,8 @@ def _load():
     lib.sldg_translate.argtypes = [vp, C.c_int, dp, C.c_size_t]
     lib.sldg_translate_dev.argtypes = [vp, C.c_int, vp, C.c_size_t]
     lib.sldg_advect.argtypes = [vp, C.c_int, C.c_double]
+    lib.sldg_advect_pair.argtypes = [vp, C.c_int, C.c_int, C.c_double]
+    lib.sldg_translate_pair_dev.argtypes = [vp, C.c_int, vp, C.c_size_t, C.c_int, vp, C.c_size_t]
     lib.sldg_compute_rho.argtypes = [vp, vp]
     lib.sldg_poisson_E.argtypes = [vp, vp]
     lib.sldg_set_E.argtypes = [vp, vp, C.c_int]
@@ -160,6 +162,16 @@ class Sldg:
 
     def advect(self, dim, dt):
         self._chk(_lib.sldg_advect(self.h, dim, float(dt)), "advect")
+
+    def advect_pair(self, dim1, dim2, dt):
+        self._chk(_lib.sldg_advect_pair(self.h, dim1, dim2, float(dt)), "advect_pair")
+
+    def translate_pair(self, dim1, shift1, dim2, shift2):
+        """Fused pair of raw sweeps; shift tables are fp64 CUDA tensors."""
+        for t in (shift1, shift2):
+            assert t.is_cuda and t.dtype == self.torch.float64 and t.is_contiguous()
+        self._chk(_lib.sldg_translate_pair_dev(self.h, dim1, shift1.data_ptr(), shift1.numel(),
+                                               dim2, shift2.data_ptr(), shift2.numel()), "translate_pair_dev")
 
     def compute_rho(self, out=True):
         """rho into the context; with out=True also returned as a new device tensor."""

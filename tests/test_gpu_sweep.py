@@ -149,3 +149,84 @@ def test_tma_and_plain_kernels_agree_bit_for_bit(monkeypatch):
         outs.append(s.get_f())
         s.close()
     assert np.array_equal(outs[0], outs[1])
+
+
+# ---------------------------------------------------------------- fused pairs (S:8(f) NEXT-1)
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("o", [1, 2, 3, 4])
+def test_fused_pair_is_bitwise_the_two_sweeps_2p2(oracle, o, dtype):
+    import torch
+    cfg = W.Config("p22", 2, 2, (11, 7, 9, 6), o, (0.0,) * 4, (11.0, 7.0, 9.0, 6.0))
+    rng = np.random.default_rng(77 + o)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
+    for (k1, k2) in ((0, 1), (2, 3)):
+        sig = []
+        for k in (k1, k2):
+            cnt = cfg.N[cfg.dx + k] if k < cfg.dx else cfg.X
+            sig.append(rng.uniform(-3.5, 3.5, cnt))
+        a = make_solver(cfg, dtype)
+        a.set_initial(f0)
+        a.translate_pair(k1, torch.from_numpy(sig[0]).cuda(), k2, torch.from_numpy(sig[1]).cuda())
+        fused = a.get_f()
+        a.close()
+        b = make_solver(cfg, dtype)
+        b.set_initial(f0)
+        b.translate(k1, sig[0])
+        b.translate(k2, sig[1])
+        seq = b.get_f()
+        b.close()
+        assert np.array_equal(fused, seq), (k1, k2)
+        ref = f0.copy()
+        oracle.translate(ref, cfg.N, cfg.order, k1, sig[0], dep_of(cfg.dx, k1))
+        oracle.translate(ref, cfg.N, cfg.order, k2, sig[1], dep_of(cfg.dx, k2))
+        assert rel_err(fused, ref) <= TOL[dtype], (k1, k2)
+
+
+def test_fused_pairs_3p3_all_legal_pairs(oracle):
+    import torch
+    cfg = W.Config("p33", 3, 3, (5, 4, 3, 4, 3, 5), 2, (0.0,) * 6, (5.0, 4.0, 3.0, 4.0, 3.0, 5.0))
+    rng = np.random.default_rng(5)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof)
+    for (k1, k2) in ((0, 1), (0, 2), (1, 2), (3, 4), (3, 5), (4, 5)):
+        sig = [rng.uniform(-2.5, 2.5, cfg.N[cfg.dx + k] if k < cfg.dx else cfg.X) for k in (k1, k2)]
+        s = make_solver(cfg, "f64")
+        s.set_initial(f0)
+        s.translate_pair(k1, torch.from_numpy(sig[0]).cuda(), k2, torch.from_numpy(sig[1]).cuda())
+        fused = s.get_f()
+        s.close()
+        ref = f0.copy()
+        oracle.translate(ref, cfg.N, cfg.order, k1, sig[0], dep_of(cfg.dx, k1))
+        oracle.translate(ref, cfg.N, cfg.order, k2, sig[1], dep_of(cfg.dx, k2))
+        assert rel_err(fused, ref) <= TOL["f64"], (k1, k2)
+
+
+def test_fused_pair_rejects_mixed_groups():
+    import torch
+    from paper_1907_08316_b200.sldg import SldgError
+    cfg = W.Config("p22", 2, 2, (4, 4, 4, 4), 2, (0.0,) * 4, (1.0,) * 4)
+    s = make_solver(cfg, "f64")
+    z = torch.zeros(cfg.N[3], dtype=torch.float64, device="cuda")
+    zx = torch.zeros(cfg.X, dtype=torch.float64, device="cuda")
+    with pytest.raises(SldgError):
+        s.translate_pair(1, z, 2, zx)          # x_2 with v_1: the v-shift depends on the x_2 node
+    with pytest.raises(SldgError):
+        s.translate_pair(1, z, 0, z)           # not ascending
+    s.close()
+
+
+def test_step_fused_equals_step_unfused_bitwise(monkeypatch):
+    cfg = W.CONFIG3.scaled((10, 8, 12, 6))
+    outs = []
+    for flag in ("0", "1"):
+        monkeypatch.setenv("SLDG_NO_FUSE", flag)
+        s = make_solver(cfg, "f64")
+        coords = [s.node_coords(d) for d in range(4)]
+        s.set_initial(W.initial_state(cfg, coords))
+        l0 = s.launch_count()
+        for _ in range(3):
+            s.step(cfg.dt)
+        outs.append((s.get_f(), s.launch_count() - l0))
+        s.close()
+    assert np.array_equal(outs[0][0], outs[1][0])
+    assert outs[0][1] < outs[1][1]             # the fused step really launches fewer sweeps
