@@ -522,8 +522,10 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
     int cps = (int)cdiv(n2, nseg);
     nseg = (int)cdiv(n2, cps);
     long threads = lines * nseg;
+    int chunk = 32;
+    while (inner1 % chunk) chunk /= 2;
     sweep_pair_kernel<T, O><<<(unsigned)cdiv(threads, 128), 128, 0, c->stream>>>(
-        in, out, inner1, n1, midN, n2, outer2, nseg, cps, c->d_m, (const T *)c->d_ab, count1, qd1, qm1,
+        in, out, inner1, n1, midN, n2, outer2, nseg, cps, chunk, c->d_m, (const T *)c->d_ab, count1, qd1, qm1,
         c->d_m2, (const T *)c->d_ab2, count2, qd2, qm2);
     LAUNCH_CHECK(c);
     c->cur ^= 1;

@@ -24,12 +24,17 @@ namespace sldg {
 template <typename T, int O>
 __global__ void __launch_bounds__(128)
 sweep_pair_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, int n1, long midN, int n2,
-                  long outer2, int nseg, int cps,
+                  long outer2, int nseg, int cps, int chunk,
                   const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
                   const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2) {
+    // thread order: `chunk` consecutive inner1 indices (lanes, coalesced), then the k1-cell c, then
+    // the remaining inner1 blocks: the two threads that read the same raw k1-cell (owners of c and
+    // c-1) sit in the same or the neighbouring block, so the second read is an L1/L2 hit.
     long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long ii = t % inner1; t /= inner1;
+    const long il = t % chunk; t /= chunk;
     const int c = (int)(t % n1); t /= n1;
+    const long ih = t % (inner1 / chunk); t /= (inner1 / chunk);
+    const long ii = ih * chunk + il;
     const long mid = t % midN; t /= midN;
     const int seg = (int)(t % nseg);
     const long oo2 = t / nseg;
@@ -63,9 +68,8 @@ sweep_pair_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, in
     if (c1 > n2) c1 = n2;
     if (c0 >= c1) return;
 
-    // k1-swept values of this thread's cell for one k2-cell: w[l2][j1]
-    auto swept_cell = [&](int cell2, T (&w)[O][O]) {
-        T r0[O][O], r1[O][O];
+    // raw values of the two k1 source cells for the O rows of one k2-cell
+    auto load_raw = [&](int cell2, T (&r0)[O][O], T (&r1)[O][O]) {
 #pragma unroll
         for (int l2 = 0; l2 < O; ++l2) {
             const long ro = ((long)cell2 * O + l2) * stride2;
@@ -75,20 +79,17 @@ sweep_pair_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, in
                 r1[l2][l] = src1[ro + l * s1];
             }
         }
+    };
+    // k1 rule on them: the O x O k1-swept values of this thread's own cell, w[l2][j1]
+    auto k1_rule = [&](const T (&r0)[O][O], const T (&r1)[O][O], T (&w)[O][O]) {
 #pragma unroll
         for (int l2 = 0; l2 < O; ++l2)
 #pragma unroll
             for (int j1 = 0; j1 < O; ++j1) w[l2][j1] = chain<T, O>(A1, B1, j1, r0[l2], r1[l2]);
     };
 
-    int is2 = c0 + m2;
-    if (is2 >= n2) is2 -= n2;
-    T w0[O][O], w1[O][O];
-    swept_cell(is2, w0);
-    T *dst = out + lin0 + (long)c0 * O * stride2;
-    for (int i2 = c0; i2 < c1; ++i2) {
-        if (++is2 == n2) is2 = 0;
-        swept_cell(is2, w1);
+    // the O x O outputs of k2-cell i2 from the window (w0 = k2 source cell i*, w1 = i*+1)
+    auto emit = [&](T *dst, const T (&w0)[O][O], const T (&w1)[O][O]) {
 #pragma unroll
         for (int j2 = 0; j2 < O; ++j2) {
 #pragma unroll
@@ -99,11 +100,39 @@ sweep_pair_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, in
                 dst[(long)j2 * stride2 + j1 * s1] = chain<T, O>(A2, B2, j2, a0, a1);
             }
         }
+    };
+
+    // Software pipeline: the raw values of the next PF k2-cells are in flight while the current
+    // cell is computed (the kernel is bound by memory latency, not by DRAM or arithmetic: ncu
+    // shows long-scoreboard stalls with DRAM at 61 % at PF = 1).  Measured at config 3 / config 4,
+    // traffic rate of the (x_1,x_2) pair: PF 1/2/3/4 = 4.9/5.7/6.1/6.0 TB/s (O = 2), PF 1/2 = 5.0/5.3 (O = 3).
+    constexpr int PF = (O <= 2) ? 3 : (O == 3 ? 2 : 1);
+    int is2 = c0 + m2;
+    if (is2 >= n2) is2 -= n2;
+    T ra[PF][O][O], rb[PF][O][O], w0[O][O], w1[O][O];
+    load_raw(is2, ra[0], rb[0]);
+    k1_rule(ra[0], rb[0], w0);
 #pragma unroll
-        for (int l = 0; l < O; ++l)
+    for (int p = 0; p < PF; ++p) {
+        if (++is2 == n2) is2 = 0;
+        if (c0 + p < c1) load_raw(is2, ra[p], rb[p]);
+    }
+    T *dst = out + lin0 + (long)c0 * O * stride2;
+    for (int i2 = c0; i2 < c1; i2 += PF) {
 #pragma unroll
-            for (int j1 = 0; j1 < O; ++j1) w0[l][j1] = w1[l][j1];
-        dst += (long)O * stride2;
+        for (int p = 0; p < PF; ++p) {
+            if (i2 + p < c1) {
+                k1_rule(ra[p], rb[p], w1);
+                if (++is2 == n2) is2 = 0;
+                if (i2 + p + PF < c1) load_raw(is2, ra[p], rb[p]);
+                emit(dst, w0, w1);
+#pragma unroll
+                for (int l = 0; l < O; ++l)
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) w0[l][j1] = w1[l][j1];
+                dst += (long)O * stride2;
+            }
+        }
     }
 }
 
