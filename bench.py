@@ -238,6 +238,38 @@ def sweep_table(torch, s, cfg, dtype, reps, warm):
     return out
 
 
+def strang_step_table(torch, Sldg, cfg, dtype, steps):
+    """Full Strang steps (sldg_step, fused sweep pairs) of a Landau config: ms per step and the
+    paper's eq. (1) style bandwidth (2(2dx+dx)+1 passes of N*sizeof(T) per step)."""
+    s = Sldg.from_config(cfg, dtype=dtype)
+    coords = [s.node_coords(d) for d in range(cfg.dx + cfg.dv)]
+    gx, gv = W.initial_factors(cfg, coords)
+    f0 = torch.outer(torch.from_numpy(gv).cuda(), torch.from_numpy(gx).cuda()).reshape(-1).to(s.tdtype)
+    s.set_initial(f0.contiguous())
+    del f0
+    for _ in range(3):
+        s.step(cfg.dt)
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    l0 = s.launch_count()
+    e0.record()
+    for _ in range(steps):
+        s.step(cfg.dt)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    es = 8 if dtype == "f64" else 4
+    passes = 2 * (3 * cfg.dx) + 1
+    mass, l2, ee = s.diagnostics()
+    out = {"ms_per_step": ms, "passes_paper_accounting": passes,
+           "gbs_paper_eq1_style": passes * cfg.ndof * es / ms / 1e6,
+           "dof_updates_per_s": 3 * cfg.dx * cfg.ndof / ms * 1e3,
+           "launches_per_step": (s.launch_count() - l0) / steps, "mass": mass, "electric_energy": ee}
+    s.close()
+    del s
+    torch.cuda.empty_cache()
+    return out
+
+
 def max_over_ranks(values, world, device):
     """Element-wise MAX of a list of floats over all ranks (timings are max-over-ranks)."""
     if world <= 1:
@@ -391,6 +423,14 @@ def run_ours(args):
             except Exception as exc:        # report, never hide
                 extras["%s-%s" % (c2.name, dt_)] = {"error": str(exc)}
         line["sweeps_other_configs"] = extras
+        steps_tab = {}
+        for name, nst in (("config3", 20), ("config5", 5)):
+            c2 = W.CONFIGS[name] if args.workload == "config4" else pick_workload(name + "/2")
+            try:
+                steps_tab[c2.name] = strang_step_table(torch, Sldg, c2, "f64", nst)
+            except Exception as exc:
+                steps_tab[c2.name] = {"error": str(exc)}
+        line["strang_steps_fused"] = steps_tab
 
     # ---- the oracle on the host cores, bounded sample (rank 0, N = 1 only)
     if world == 1 and rank == 0 and not args.no_cpu_baseline:

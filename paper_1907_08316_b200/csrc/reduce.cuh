@@ -15,7 +15,7 @@ namespace sldg {
 
 // part_rho[split][x] = sum_{v in split} W_v f[v][x];  part_s2 likewise with f^2 (if WITH_S2)
 template <typename T, int VEC, bool WITH_S2, int UB>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(128)
 vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
                     const double *__restrict__ Wv, double *__restrict__ part_rho,
                     double *__restrict__ part_s2) {

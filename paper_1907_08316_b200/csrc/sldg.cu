@@ -43,13 +43,23 @@ struct sldg_ctx {
     // device tables
     double *d_coef = nullptr;          // A/B polynomial coefficients [2][o][o][2o]
     double *d_coords[SLDG_MAX_DIM] = {nullptr};   // node coordinates per dimension
-    long tab_cap = 0;                  // capacity (entries) of the sweep tables
-    double *d_sigma = nullptr;         // [tab_cap]
-    int *d_m = nullptr;                // [tab_cap]
-    void *d_ab = nullptr;              // [2 o^2][tab_cap] of T
-    double *d_sigma2 = nullptr;        // second table set (second sweep of a fused pair)
-    int *d_m2 = nullptr;
-    void *d_ab2 = nullptr;
+    long tab_cap = 0;                  // capacity (entries) of the general sweep tables
+    // Sweep tables (a-1).  Storage: gen[0..1] (capacity tab_cap: v-sweeps, raw sldg_translate calls,
+    // the two halves of a fused pair) and xt[a] (capacity N_{v_a}: the physics x_a sweep, whose
+    // shifts c_v*tau/h never change, cached per tau so that sigma + assembly run once, not per step).
+    struct Tab {
+        double *sigma = nullptr;       // [cap] shift in cell widths
+        int *m = nullptr;              // [cap] cell offset mod n
+        void *ab = nullptr;            // [2 o^2][cap] of T
+        double tau = 0.0;
+        bool valid = false;            // m/ab hold the assembled table for `tau`
+    };
+    Tab gen[2], xt[3];
+    // the table set(s) the next sweep launch reads: aliases into gen[] / xt[]
+    double *d_sigma = nullptr, *d_sigma2 = nullptr;
+    int *d_m = nullptr, *d_m2 = nullptr;
+    void *d_ab = nullptr, *d_ab2 = nullptr;
+    bool skip_asm1 = false, skip_asm2 = false;
     double *d_Wv = nullptr, *d_Wx = nullptr;      // quadrature weights over v-nodes / x-nodes
     double *d_rho = nullptr, *d_s2 = nullptr, *d_E = nullptr;   // [X], [X], [dx][X]
     int max_splits = 1;
@@ -106,8 +116,8 @@ cudaError_t dalloc(P **p, size_t count) {
 void free_tables(sldg_ctx *c) {
     cudaFree(c->d_coef);
     for (int d = 0; d < SLDG_MAX_DIM; ++d) cudaFree(c->d_coords[d]);
-    cudaFree(c->d_sigma); cudaFree(c->d_m); cudaFree(c->d_ab);
-    cudaFree(c->d_sigma2); cudaFree(c->d_m2); cudaFree(c->d_ab2);
+    for (auto &t : c->gen) { cudaFree(t.sigma); cudaFree(t.m); cudaFree(t.ab); }
+    for (auto &t : c->xt) { cudaFree(t.sigma); cudaFree(t.m); cudaFree(t.ab); }
     cudaFree(c->d_Wv); cudaFree(c->d_Wx);
     cudaFree(c->d_rho); cudaFree(c->d_s2); cudaFree(c->d_E);
     cudaFree(c->d_part); cudaFree(c->d_scal);
@@ -211,12 +221,18 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         if (c->N[d] > maxN) maxN = c->N[d];
     }
     c->tab_cap = c->X > maxN ? c->X : maxN;
-    CREATE_TRY(dalloc(&c->d_sigma, c->tab_cap));
-    CREATE_TRY(dalloc(&c->d_m, c->tab_cap));
-    CREATE_TRY(cudaMalloc(&c->d_ab, (size_t)2 * order * order * c->tab_cap * c->esize));
-    CREATE_TRY(dalloc(&c->d_sigma2, c->tab_cap));
-    CREATE_TRY(dalloc(&c->d_m2, c->tab_cap));
-    CREATE_TRY(cudaMalloc(&c->d_ab2, (size_t)2 * order * order * c->tab_cap * c->esize));
+    for (auto &t : c->gen) {
+        CREATE_TRY(dalloc(&t.sigma, c->tab_cap));
+        CREATE_TRY(dalloc(&t.m, c->tab_cap));
+        CREATE_TRY(cudaMalloc(&t.ab, (size_t)2 * order * order * c->tab_cap * c->esize));
+    }
+    for (int a = 0; a < dx; ++a) {
+        sldg_ctx::Tab &t = c->xt[a];
+        long cap = c->N[dx + a];
+        CREATE_TRY(dalloc(&t.sigma, cap));
+        CREATE_TRY(dalloc(&t.m, cap));
+        CREATE_TRY(cudaMalloc(&t.ab, (size_t)2 * order * order * cap * c->esize));
+    }
 
     // quadrature weights W_v = prod_a h_va w_ja (v_1 fastest), W_x likewise
     {
@@ -374,7 +390,7 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
     const T *in = (const T *)c->buf[c->cur];
     T *out = (T *)c->buf[c->cur ^ 1];
     // a-1
-    {
+    if (!c->skip_asm1) {
         int block = 128;
         size_t sh = (size_t)2 * O * O * 2 * O * 2 * sizeof(double);
         assemble_ab_kernel<T><<<(unsigned)cdiv(count, block), block, sh, c->stream>>>(
@@ -491,12 +507,16 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
     T *out = (T *)c->buf[c->cur ^ 1];
     int block = 128;
     size_t sh = (size_t)2 * O * O * 2 * O * 2 * sizeof(double);
-    assemble_ab_kernel<T><<<(unsigned)cdiv(count1, block), block, sh, c->stream>>>(
-        c->d_sigma, count1, O, n1, c->d_coef, c->d_m, (T *)c->d_ab);
-    LAUNCH_CHECK(c);
-    assemble_ab_kernel<T><<<(unsigned)cdiv(count2, block), block, sh, c->stream>>>(
-        c->d_sigma2, count2, O, n2, c->d_coef, c->d_m2, (T *)c->d_ab2);
-    LAUNCH_CHECK(c);
+    if (!c->skip_asm1) {
+        assemble_ab_kernel<T><<<(unsigned)cdiv(count1, block), block, sh, c->stream>>>(
+            c->d_sigma, count1, O, n1, c->d_coef, c->d_m, (T *)c->d_ab);
+        LAUNCH_CHECK(c);
+    }
+    if (!c->skip_asm2) {
+        assemble_ab_kernel<T><<<(unsigned)cdiv(count2, block), block, sh, c->stream>>>(
+            c->d_sigma2, count2, O, n2, c->d_coef, c->d_m2, (T *)c->d_ab2);
+        LAUNCH_CHECK(c);
+    }
     long inner1 = 1, midN = 1, outer2 = 1;
     for (int d = 0; d < k1; ++d) inner1 *= c->N[d];
     for (int d = k1 + 1; d < k2; ++d) midN *= c->N[d];
@@ -546,6 +566,12 @@ int run_pair(sldg_ctx *c, int k1, int k2, long count1, long count2) {
     return fail(c, SLDG_ERR_UNSUPPORTED, "order %d not instantiated", c->o);
 }
 
+// point table slot 1 or 2 at a storage set; `assembled` = its m/ab are already valid
+void use_tab(sldg_ctx *c, int slot, sldg_ctx::Tab &t, bool assembled) {
+    if (slot == 1) { c->d_sigma = t.sigma; c->d_m = t.m; c->d_ab = t.ab; c->skip_asm1 = assembled; }
+    else { c->d_sigma2 = t.sigma; c->d_m2 = t.m; c->d_ab2 = t.ab; c->skip_asm2 = assembled; }
+}
+
 long sweep_count(const sldg_ctx *c, int dim) { return dim < c->dx ? c->N[c->dx + dim] : c->X; }
 
 }  // namespace
@@ -554,6 +580,7 @@ extern "C" int sldg_translate(sldg_ctx *c, int dim, const double *shift, size_t 
     if (!c || !shift || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
     if ((long)count != sweep_count(c, dim))
         return fail(c, SLDG_ERR_ARG, "sldg_translate: dim %d needs %ld shifts, got %zu", dim, sweep_count(c, dim), count);
+    use_tab(c, 1, c->gen[0], false);
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift, count * sizeof(double), cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));   // the host array may be reused by the caller
     return run_sweep(c, dim, (long)count);
@@ -563,25 +590,34 @@ extern "C" int sldg_translate_dev(sldg_ctx *c, int dim, const double *shift, siz
     if (!c || !shift || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
     if ((long)count != sweep_count(c, dim))
         return fail(c, SLDG_ERR_ARG, "sldg_translate_dev: dim %d needs %ld shifts, got %zu", dim, sweep_count(c, dim), count);
+    use_tab(c, 1, c->gen[0], false);
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift, count * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     return run_sweep(c, dim, (long)count);
 }
 
 namespace {
-// sigma of a physics sweep (D:O3, D:R4) into `sigma` on the stream
-int fill_physics_sigma(sldg_ctx *c, int dim, double dt, double *sigma) {
+// Table of a physics sweep (D:O3, D:R4) into slot 1 or 2: fills sigma on the stream unless the
+// cached x-table for this tau is still valid.
+int physics_tab(sldg_ctx *c, int slot, int dim, double dt) {
     long count = sweep_count(c, dim);
     int block = 256;
     if (dim < c->dx) {
+        sldg_ctx::Tab &t = c->xt[dim];
+        if (t.valid && t.tau == dt) { use_tab(c, slot, t, true); return SLDG_OK; }
+        use_tab(c, slot, t, false);
         int va = c->dx + dim;
         sigma_from_coords_kernel<<<(unsigned)cdiv(count, block), block, 0, c->stream>>>(
-            c->d_coords[va], count, dt, c->h[dim], sigma);
+            c->d_coords[va], count, dt, c->h[dim], t.sigma);
+        t.tau = dt;
+        t.valid = true;                 // the assembly is enqueued by the sweep that follows
     } else {
         int a = dim - c->dx;
         if (a >= c->dx) return fail(c, SLDG_ERR_ARG, "sldg_advect: v_%d has no field component (dx = %d)", a + 1, c->dx);
         if (!c->have_E) return fail(c, SLDG_ERR_STATE, "sldg_advect: no E stored (call sldg_poisson_E or sldg_set_E)");
+        sldg_ctx::Tab &t = c->gen[slot - 1];
+        use_tab(c, slot, t, false);
         sigma_from_E_kernel<<<(unsigned)cdiv(count, block), block, 0, c->stream>>>(
-            c->d_E + (long)a * c->X, count, dt, c->h[dim], sigma);
+            c->d_E + (long)a * c->X, count, dt, c->h[dim], t.sigma);
     }
     LAUNCH_CHECK(c);
     return SLDG_OK;
@@ -595,7 +631,7 @@ bool pair_ok(const sldg_ctx *c, int d1, int d2) {
 
 extern "C" int sldg_advect(sldg_ctx *c, int dim, double dt) {
     if (!c || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
-    int rc = fill_physics_sigma(c, dim, dt, c->d_sigma);
+    int rc = physics_tab(c, 1, dim, dt);
     if (rc) return rc;
     return run_sweep(c, dim, sweep_count(c, dim));
 }
@@ -604,9 +640,9 @@ extern "C" int sldg_advect_pair(sldg_ctx *c, int dim1, int dim2, double dt) {
     if (!c) return SLDG_ERR_ARG;
     if (!pair_ok(c, dim1, dim2))
         return fail(c, SLDG_ERR_ARG, "sldg_advect_pair: need dim1 < dim2, both x- or both v-dimensions");
-    int rc = fill_physics_sigma(c, dim1, dt, c->d_sigma);
+    int rc = physics_tab(c, 1, dim1, dt);
     if (rc) return rc;
-    if ((rc = fill_physics_sigma(c, dim2, dt, c->d_sigma2))) return rc;
+    if ((rc = physics_tab(c, 2, dim2, dt))) return rc;
     return run_pair(c, dim1, dim2, sweep_count(c, dim1), sweep_count(c, dim2));
 }
 
@@ -617,6 +653,8 @@ extern "C" int sldg_translate_pair_dev(sldg_ctx *c, int dim1, const double *shif
         return fail(c, SLDG_ERR_ARG, "sldg_translate_pair_dev: need dim1 < dim2, both x- or both v-dimensions");
     if ((long)count1 != sweep_count(c, dim1) || (long)count2 != sweep_count(c, dim2))
         return fail(c, SLDG_ERR_ARG, "sldg_translate_pair_dev: wrong shift counts");
+    use_tab(c, 1, c->gen[0], false);
+    use_tab(c, 2, c->gen[1], false);
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift1, count1 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma2, shift2, count2 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     return run_pair(c, dim1, dim2, (long)count1, (long)count2);
@@ -627,13 +665,12 @@ extern "C" int sldg_translate_pair_dev(sldg_ctx *c, int dim1, const double *shif
 // ------------------------------------------------------------------------------------------
 namespace {
 
-template <typename T, int VEC, bool S2>
-void launch_vsum(sldg_ctx *c, int splits, long vps) {
-    int block = 128;
+template <typename T, int VEC, bool S2, int UB>
+void launch_vsum(sldg_ctx *c, int splits, long vps, int block) {
     long xv = c->X / VEC;
     if (xv < block) block = (int)(cdiv(xv, 32) * 32);
     dim3 grid((unsigned)cdiv(xv, block), (unsigned)splits);
-    vsum_partial_kernel<T, VEC, S2, 8><<<grid, block, 0, c->stream>>>(
+    vsum_partial_kernel<T, VEC, S2, UB><<<grid, block, 0, c->stream>>>(
         (const T *)c->buf[c->cur], c->X, c->V, vps, c->d_Wv, c->d_part,
         c->d_part + (size_t)c->max_splits * c->X);
 }
@@ -650,12 +687,14 @@ int run_vsum(sldg_ctx *c, double *rho_copy) {
     // canonical order with fp64 multiply-then-add -- the order D:O4 states.  rho + 1 is a
     // difference of O(1) sums (D:R11), so the summation order is visible at 1e-13 relative in E
     // when the perturbation is 1e-3; large problems need the splits for parallelism.
-    if (c->V * c->X <= (1L << 23)) s = 1;
+    const bool small = c->V * c->X <= (1L << 23);
+    if (small) s = 1;
     long vps = cdiv(c->V, s);
     int splits = (int)cdiv(c->V, vps);
-    if (vec == VMAX) launch_vsum<T, VMAX, S2>(c, splits, vps);
-    else if (vec == 2) launch_vsum<T, 2, S2>(c, splits, vps);
-    else launch_vsum<T, 1, S2>(c, splits, vps);
+    if (small) launch_vsum<T, 1, S2, 32>(c, splits, vps, 32);     // thread per x, 32 rows in flight
+    else if (vec == VMAX) launch_vsum<T, VMAX, S2, 8>(c, splits, vps, 128);
+    else if (vec == 2) launch_vsum<T, 2, S2, 8>(c, splits, vps, 128);
+    else launch_vsum<T, 1, S2, 8>(c, splits, vps, 128);
     LAUNCH_CHECK(c);
     int block = 256;
     vsum_final_kernel<<<(unsigned)cdiv(c->X, block), block, 0, c->stream>>>(
@@ -679,9 +718,9 @@ int apply_along(sldg_ctx *c, const double *in_re, const double *in_im, long *sha
     long inner = 1, outer = 1, cols = shape[b];
     for (int d = 0; d < b; ++d) inner *= shape[d];
     for (int d = b + 1; d < nd; ++d) outer *= shape[d];
-    long total = outer * rows * inner;
-    int block = 128;
-    cplx_apply_kernel<IN_REAL, OUT_REAL><<<(unsigned)cdiv(total, block), block, 0, c->stream>>>(
+    long total = outer * rows * inner;             // one warp per output element
+    int block = 256;
+    cplx_apply_kernel<IN_REAL, OUT_REAL><<<(unsigned)cdiv(total * 32, block), block, 0, c->stream>>>(
         in_re, in_im, outer, cols, inner, M, rows, out_re, out_im);
     LAUNCH_CHECK(c);
     shape[b] = rows;
