@@ -97,6 +97,13 @@ int oracle_diagnostics_f32(const float *f, int dx, int dv, const int *cells, int
                            const double *lo, const double *hi,
                            double *mass, double *l2, double *ee);
 
+/* S:8(f) NEXT-4 (Fig. 15): momentum[a] = int int v_a f (a < dv) and
+ * kinetic = 1/2 int int |v|^2 f by Gauss quadrature on the nodes, iterated sums (R12). */
+int oracle_moments_f64(const double *f, int dx, int dv, const int *cells, int o,
+                       const double *lo, const double *hi, double *momentum, double *kinetic);
+int oracle_moments_f32(const float *f, int dx, int dv, const int *cells, int o,
+                       const double *lo, const double *hi, double *momentum, double *kinetic);
+
 /* threads the sweeps/reductions will use (OpenMP over lines), for the bench report */
 int oracle_num_threads(void);
 

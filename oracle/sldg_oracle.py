@@ -43,6 +43,7 @@ def _load():
         getattr(lib, "oracle_rho_" + suf).argtypes = [pt] + grid + [_pd]
         getattr(lib, "oracle_step_" + suf).argtypes = [pt] + grid + [C.c_double]
         getattr(lib, "oracle_diagnostics_" + suf).argtypes = [pt] + grid + [C.POINTER(C.c_double)] * 3
+        getattr(lib, "oracle_moments_" + suf).argtypes = [pt] + grid + [_pd, C.POINTER(C.c_double)]
     _lib = lib
     return lib
 
@@ -160,6 +161,12 @@ class Grid:
     def step(self, f, dt):
         _check(getattr(_load(), "oracle_step_" + _suf(f))(f, *self._args(), float(dt)), "step")
         return f
+
+    def moments(self, f):
+        """(momentum[dv], kinetic energy) -- NEXT-4 invariants."""
+        P, k = np.zeros(self.dv), C.c_double()
+        _check(getattr(_load(), "oracle_moments_" + _suf(f))(f, *self._args(), P, C.byref(k)), "moments")
+        return P, k.value
 
     def diagnostics(self, f):
         m, l2, ee = C.c_double(), C.c_double(), C.c_double()
