@@ -134,6 +134,12 @@ int sldg_step(sldg_ctx *ctx, double dt);
  * output pointers (host) may be NULL. */
 int sldg_diagnostics(sldg_ctx *ctx, double *mass, double *l2, double *electric_energy);
 
+/* S:8(f) NEXT-4 ("physical invariants", P:224 momentum conservation, Fig. 15 kinetic / total
+ * energy): momentum[a] = int int v_a f dx dv for a < dv (host array of dv doubles) and
+ * kinetic_energy = 1/2 int int |v|^2 f dx dv from the current f; one read of f; synchronises the
+ * stream.  Either pointer may be NULL.  Total energy = kinetic_energy + electric_energy. */
+int sldg_moments(sldg_ctx *ctx, double *momentum, double *kinetic_energy);
+
 /* Number of kernels this context has launched since sldg_create (bench "gpu_launches"). */
 unsigned long long sldg_launch_count(const sldg_ctx *ctx);
 

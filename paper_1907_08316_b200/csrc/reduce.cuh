@@ -121,3 +121,75 @@ scalars_kernel(const double *__restrict__ rho, const double *__restrict__ s2,
 }
 
 }  // namespace sldg
+
+namespace sldg {
+
+// S:8(f) NEXT-4 (Fig. 15): velocity moments per x-node,
+//   part[a][split][x] = sum_v v_a W_v f[v][x]  (a < DV),   part[DV][split][x] = sum_v |v|^2 W_v f[v][x],
+// one read of f, fp64 accumulators, same split structure as the rho pass.
+template <typename T, int VEC, int DV>
+__global__ void __launch_bounds__(128)
+vmoment_partial_kernel(const T *__restrict__ f, long X, long V, long vps, int nsplit_cap,
+                       const double *__restrict__ Wv, const double *__restrict__ va /* [DV][V] */,
+                       const double *__restrict__ v2, double *__restrict__ part) {
+    using Vt = Vec<T, VEC>;
+    const long xv = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long x = xv * VEC;
+    if (x >= X) return;
+    const long split = blockIdx.y;
+    const long v0 = split * vps;
+    long v1 = v0 + vps;
+    if (v1 > V) v1 = V;
+    double acc[DV + 1][VEC];
+#pragma unroll
+    for (int k = 0; k <= DV; ++k)
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) acc[k][e] = 0.0;
+    const T *p = f + v0 * X + x;
+#pragma unroll 4
+    for (long v = v0; v < v1; ++v) {
+        Vt u = *reinterpret_cast<const Vt *>(p);
+        const double w = Wv[v], s2 = v2[v];
+        double c[DV];
+#pragma unroll
+        for (int a = 0; a < DV; ++a) c[a] = va[(long)a * V + v];
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) {
+            const double wf = w * (double)u.v[e];
+#pragma unroll
+            for (int a = 0; a < DV; ++a) acc[a][e] += c[a] * wf;
+            acc[DV][e] += s2 * wf;
+        }
+        p += X;
+    }
+#pragma unroll
+    for (int k = 0; k <= DV; ++k)
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) part[((long)k * nsplit_cap + split) * X + x + e] = acc[k][e];
+}
+
+// out[k] = sum_x W_x sum_split part[k][split][x], k < nk (one block of 1024 threads, fixed order)
+__global__ void __launch_bounds__(1024)
+moments_final_kernel(const double *__restrict__ part, const double *__restrict__ Wx, long X, int splits,
+                     int nsplit_cap, int nk, double *__restrict__ out) {
+    __shared__ double sm[32];
+    for (int k = 0; k < nk; ++k) {
+        double a = 0.0;
+        for (long x = threadIdx.x; x < X; x += blockDim.x) {
+            double s = 0.0;
+            for (int sp = 0; sp < splits; ++sp) s += part[((long)k * nsplit_cap + sp) * X + x];
+            a += Wx[x] * s;
+        }
+        a = warp_sum(a);
+        const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+        if (lane == 0) sm[wid] = a;
+        __syncthreads();
+        if (wid == 0) {
+            a = warp_sum(sm[lane]);
+            if (lane == 0) out[k] = a;
+        }
+        __syncthreads();
+    }
+}
+
+}  // namespace sldg

@@ -61,10 +61,11 @@ struct sldg_ctx {
     void *d_ab = nullptr, *d_ab2 = nullptr;
     bool skip_asm1 = false, skip_asm2 = false;
     double *d_Wv = nullptr, *d_Wx = nullptr;      // quadrature weights over v-nodes / x-nodes
+    double *d_va = nullptr, *d_v2 = nullptr;      // per v-node: coordinates v_a [dv][V] and |v|^2 [V]
     double *d_rho = nullptr, *d_s2 = nullptr, *d_E = nullptr;   // [X], [X], [dx][X]
     int max_splits = 1;
-    double *d_part = nullptr;          // [2][max_splits][X]
-    double *d_scal = nullptr;          // [3]
+    double *d_part = nullptr;          // [4][max_splits][X]
+    double *d_scal = nullptr;          // [8]
     // Poisson
     long K[3] = {1, 1, 1}, Mmax[3] = {0, 0, 0}, KK = 1;
     double2 *d_F[3] = {nullptr, nullptr, nullptr}, *d_G[3] = {nullptr, nullptr, nullptr};
@@ -118,7 +119,7 @@ void free_tables(sldg_ctx *c) {
     for (int d = 0; d < SLDG_MAX_DIM; ++d) cudaFree(c->d_coords[d]);
     for (auto &t : c->gen) { cudaFree(t.sigma); cudaFree(t.m); cudaFree(t.ab); }
     for (auto &t : c->xt) { cudaFree(t.sigma); cudaFree(t.m); cudaFree(t.ab); }
-    cudaFree(c->d_Wv); cudaFree(c->d_Wx);
+    cudaFree(c->d_Wv); cudaFree(c->d_Wx); cudaFree(c->d_va); cudaFree(c->d_v2);
     cudaFree(c->d_rho); cudaFree(c->d_s2); cudaFree(c->d_E);
     cudaFree(c->d_part); cudaFree(c->d_scal);
     for (int a = 0; a < 3; ++a) { cudaFree(c->d_F[a]); cudaFree(c->d_G[a]); }
@@ -253,6 +254,24 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
             }
             Wx[x] = W;
         }
+        {   // v-node coordinates and |v|^2 for the moment pass
+            std::vector<double> va((size_t)dv * c->V), v2(c->V);
+            std::vector<std::vector<double>> cv(dv);
+            for (int a = 0; a < dv; ++a) host_node_coords(c, dx + a, cv[a]);
+            for (long v = 0; v < c->V; ++v) {
+                long rem = v; double s2 = 0.0;
+                for (int a = 0; a < dv; ++a) {
+                    long p = rem % c->N[dx + a]; rem /= c->N[dx + a];
+                    va[(size_t)a * c->V + v] = cv[a][p];
+                    s2 += cv[a][p] * cv[a][p];
+                }
+                v2[v] = s2;
+            }
+            CREATE_TRY(dalloc(&c->d_va, va.size()));
+            CREATE_TRY(dalloc(&c->d_v2, v2.size()));
+            CREATE_TRY(cudaMemcpy(c->d_va, va.data(), va.size() * sizeof(double), cudaMemcpyHostToDevice));
+            CREATE_TRY(cudaMemcpy(c->d_v2, v2.data(), v2.size() * sizeof(double), cudaMemcpyHostToDevice));
+        }
         CREATE_TRY(dalloc(&c->d_Wv, Wv.size()));
         CREATE_TRY(dalloc(&c->d_Wx, Wx.size()));
         CREATE_TRY(cudaMemcpy(c->d_Wv, Wv.data(), Wv.size() * sizeof(double), cudaMemcpyHostToDevice));
@@ -263,7 +282,7 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
     CREATE_TRY(dalloc(&c->d_E, c->X * dx));
     CREATE_TRY(cudaMemset(c->d_E, 0, c->X * dx * sizeof(double)));
     CREATE_TRY(cudaMemset(c->d_s2, 0, c->X * sizeof(double)));
-    CREATE_TRY(dalloc(&c->d_scal, 3));
+    CREATE_TRY(dalloc(&c->d_scal, 8));
     {
         // enough v-splits that X/VEC * splits threads fill the machine (about 2 waves of 2048/SM)
         long target = (long)c->sm_count * 2048 * 2;
@@ -274,7 +293,7 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         if (s < 1) s = 1;
         if (s > 1024) s = 1024;
         c->max_splits = (int)s;
-        CREATE_TRY(dalloc(&c->d_part, (size_t)2 * c->max_splits * c->X));
+        CREATE_TRY(dalloc(&c->d_part, (size_t)4 * c->max_splits * c->X));
     }
 
     // Poisson: dense DFT matrices per x-dimension (D:R6)
@@ -813,6 +832,51 @@ extern "C" int sldg_step(sldg_ctx *c, double dt) {
     if ((rc = run_poisson(c, nullptr))) return rc;
     if ((rc = advect_group(c, c->dx, c->dx, dt))) return rc;
     if ((rc = advect_group(c, 0, c->dx, 0.5 * dt))) return rc;
+    return SLDG_OK;
+}
+
+namespace {
+template <typename T, int VEC, int DV>
+void launch_vmoment(sldg_ctx *c, int splits, long vps) {
+    int block = 128;
+    long xv = c->X / VEC;
+    if (xv < block) block = (int)(cdiv(xv, 32) * 32);
+    dim3 grid((unsigned)cdiv(xv, block), (unsigned)splits);
+    vmoment_partial_kernel<T, VEC, DV><<<grid, block, 0, c->stream>>>(
+        (const T *)c->buf[c->cur], c->X, c->V, vps, c->max_splits, c->d_Wv, c->d_va, c->d_v2, c->d_part);
+}
+template <typename T>
+int run_moments(sldg_ctx *c) {
+    constexpr int VMAX = 16 / (int)sizeof(T);
+    const int vec = (c->X % VMAX == 0) ? VMAX : 1;
+    long target = (long)c->sm_count * 2048 * 2;
+    long s = cdiv(target, c->X / vec > 0 ? c->X / vec : 1);
+    if (s > c->max_splits) s = c->max_splits;
+    if (s < 1) s = 1;
+    long vps = cdiv(c->V, s);
+    int splits = (int)cdiv(c->V, vps);
+#define MOM_CASE(DV)                                                   \
+    if (vec == VMAX) launch_vmoment<T, VMAX, DV>(c, splits, vps);      \
+    else launch_vmoment<T, 1, DV>(c, splits, vps);
+    if (c->dv == 1) { MOM_CASE(1) } else if (c->dv == 2) { MOM_CASE(2) } else { MOM_CASE(3) }
+#undef MOM_CASE
+    LAUNCH_CHECK(c);
+    moments_final_kernel<<<1, 1024, 0, c->stream>>>(c->d_part, c->d_Wx, c->X, splits, c->max_splits, c->dv + 1,
+                                                    c->d_scal + 3);
+    LAUNCH_CHECK(c);
+    return SLDG_OK;
+}
+}  // namespace
+
+extern "C" int sldg_moments(sldg_ctx *c, double *momentum, double *kinetic) {
+    if (!c) return SLDG_ERR_ARG;
+    int rc = c->dtype == SLDG_F64 ? run_moments<double>(c) : run_moments<float>(c);
+    if (rc) return rc;
+    double h[4];
+    CUDA_TRY(c, cudaMemcpyAsync(h, c->d_scal + 3, (c->dv + 1) * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    if (momentum) for (int a = 0; a < c->dv; ++a) momentum[a] = h[a];
+    if (kinetic) *kinetic = 0.5 * h[c->dv];
     return SLDG_OK;
 }
 

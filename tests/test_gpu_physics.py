@@ -143,3 +143,54 @@ def test_config5_reduced_twin(oracle):
     got, ref, tg, tr = _run_config(oracle, cfg, "f64", cfg.steps)
     assert rel_err(got, ref) <= TOL["f64"]
     _check_traces(tg, tr, TOL["f64"])
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(1, 1, (9, 7)), (2, 2, (6, 5, 4, 7)), (3, 3, (4, 3, 5, 3, 4, 3)),
+                                   (1, 3, (8, 5, 4, 3)), (2, 3, (5, 4, 3, 4, 3))])
+def test_moments_match_oracle(oracle, shape, dtype):
+    """NEXT-4: momentum and kinetic energy (sldg_moments) against the oracle."""
+    dx, dv, cells = shape
+    o = 3 if dx < 3 else 2
+    lo = (0.0,) * dx + (-4.0, -3.0, -5.0)[:dv]
+    hi = tuple(2 * np.pi * (1 + 0.5 * a) for a in range(dx)) + (4.5, 3.5, 4.0)[:dv]
+    cfg = W.Config("m", dx, dv, cells, o, lo, hi)
+    rng = np.random.default_rng(9)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
+    s = make_solver(cfg, dtype)
+    s.set_initial(f0)
+    P, K = s.moments()
+    Pr, Kr = _grid(oracle, cfg).moments(f0)
+    s.close()
+    assert np.max(np.abs(P - Pr)) <= 1e-13 * np.max(np.abs(Pr)) + 1e-13 * abs(Kr)
+    assert abs(K - Kr) <= 1e-13 * abs(Kr)
+
+
+def test_config1_momentum_and_total_energy_on_the_gpu(oracle):
+    cfg = W.CONFIG1
+    s = make_solver(cfg, "f64")
+    s.set_initial(W.initial_state(cfg, _coords(oracle, cfg)))
+    P0, K0 = s.moments()
+    ee0 = s.diagnostics()[2]
+    for _ in range(50):
+        s.step(cfg.dt)
+    P1, K1 = s.moments()
+    ee1 = s.diagnostics()[2]
+    s.close()
+    assert abs(P1[0]) < 1e-9 and abs((K1 + ee1) - (K0 + ee0)) < 1e-5 * (K0 + ee0)
+
+
+# ---------------------------------------------------------------- NEXT-3: mixed d_x != d_v (P:200-212)
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(1, 3, (10, 6, 5, 4)), (2, 3, (6, 5, 6, 4, 5)), (1, 2, (12, 7, 5))])
+def test_mixed_dimension_steps(oracle, shape, dtype):
+    """1+3 D and 2+3 D (the paper's section 7 set-ups) and 1+2 D: full Strang steps vs the oracle.
+    Only v_1..v_dx are accelerated (E has d_x components); the remaining v are parameters."""
+    dx, dv, cells = shape
+    lo = (0.0,) * dx + (-6.0,) * dv
+    hi = (4 * np.pi,) * dx + (6.0,) * dv
+    cfg = W.Config("mix", dx, dv, cells, 2, lo, hi, dt=0.1, steps=4, kind="landau", eps=0.05, k=0.5)
+    got, ref, tg, tr = _run_config(oracle, cfg, dtype, cfg.steps)
+    assert rel_err(got, ref) <= TOL[dtype]
+    _check_traces(tg, tr, max(TOL[dtype], 1e-11))
