@@ -54,7 +54,7 @@ typedef enum {
 } sldg_status;
 
 #define SLDG_MAX_DIM 6
-#define SLDG_MAX_ORDER 4
+#define SLDG_MAX_ORDER 6
 
 /* Create a solver context (template parameters (d_x, d_v, o) become run-time here).
  *   dx, dv      1..3 each, dv >= dx (E has dx components and accelerates v_1..v_dx)

@@ -107,8 +107,14 @@ int oracle_node_coords(int n_cells, int o, double lo, double hi, double *c) {
 void oracle_shift_split(double sigma, long *m, double *theta) {
     double delta = -sigma;
     double fl = floor(delta);
+    double th = delta - fl;
+    /* R3: theta lies in [0,1).  For a tiny negative delta (|delta| < 2^-54: e.g. E = -1e-18 of
+     * rounding noise at a node where the field vanishes) the subtraction rounds to exactly 1.0;
+     * the translation is continuous across integers (A(1) = 0, B(1) = I equals the next cell with
+     * A(0) = I, B(0) = 0), so that case IS the integer shift fl + 1 with theta = 0. */
+    if (th >= 1.0) { fl += 1.0; th = 0.0; }
     *m = (long)fl;
-    *theta = delta - fl;
+    *theta = th;
 }
 
 /* ---- O2: A(theta), B(theta) --------------------------------------------- */

@@ -510,6 +510,8 @@ int run_sweep_o(sldg_ctx *c, int dim, long count) {
     case 2: return run_sweep_t<T, 2>(c, dim, count);
     case 3: return run_sweep_t<T, 3>(c, dim, count);
     case 4: return run_sweep_t<T, 4>(c, dim, count);
+    case 5: return run_sweep_t<T, 5>(c, dim, count);
+    case 6: return run_sweep_t<T, 6>(c, dim, count);
     }
     return fail(c, SLDG_ERR_UNSUPPORTED, "order %d not instantiated", c->o);
 }
@@ -659,6 +661,10 @@ extern "C" int sldg_advect_pair(sldg_ctx *c, int dim1, int dim2, double dt) {
     if (!c) return SLDG_ERR_ARG;
     if (!pair_ok(c, dim1, dim2))
         return fail(c, SLDG_ERR_ARG, "sldg_advect_pair: need dim1 < dim2, both x- or both v-dimensions");
+    if (c->o > 4) {                      // the fused kernel is instantiated for o <= 4 (registers)
+        int r1 = sldg_advect(c, dim1, dt);
+        return r1 ? r1 : sldg_advect(c, dim2, dt);
+    }
     int rc = physics_tab(c, 1, dim1, dt);
     if (rc) return rc;
     if ((rc = physics_tab(c, 2, dim2, dt))) return rc;
@@ -672,6 +678,10 @@ extern "C" int sldg_translate_pair_dev(sldg_ctx *c, int dim1, const double *shif
         return fail(c, SLDG_ERR_ARG, "sldg_translate_pair_dev: need dim1 < dim2, both x- or both v-dimensions");
     if ((long)count1 != sweep_count(c, dim1) || (long)count2 != sweep_count(c, dim2))
         return fail(c, SLDG_ERR_ARG, "sldg_translate_pair_dev: wrong shift counts");
+    if (c->o > 4) {
+        int r1 = sldg_translate_dev(c, dim1, shift1, count1);
+        return r1 ? r1 : sldg_translate_dev(c, dim2, shift2, count2);
+    }
     use_tab(c, 1, c->gen[0], false);
     use_tab(c, 2, c->gen[1], false);
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift1, count1 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));

@@ -47,7 +47,8 @@ __global__ void assemble_ab_kernel(const double *__restrict__ sigma, long count,
     if (q >= count) return;
     double delta = -sigma[q];
     double fl = floor(delta);
-    double theta = delta - fl;                     // exact (Sterbenz / same binade)
+    double theta = delta - fl;
+    if (theta >= 1.0) { fl += 1.0; theta = 0.0; }  // |delta| < 2^-54 negative: rounds to 1, is the next integer shift (D:R3)
     // m mod n without overflow for large |shift|: fmod on the (integer-valued) double
     double mm = fmod(fl, (double)n);
     if (mm < 0.0) mm += (double)n;
@@ -209,7 +210,7 @@ sweep_x1_kernel(const T *__restrict__ in, T *__restrict__ out, int n, long ngrou
     const int bg = blockIdx.x % blocks_per_group;
     if (g >= ngroups) return;
     const long q = g % qmod;
-    if (threadIdx.x < 2 * O * O) s_ab[threadIdx.x] = ab[(long)threadIdx.x * count + q];
+    for (int e = threadIdx.x; e < 2 * O * O; e += blockDim.x) s_ab[e] = ab[(long)e * count + q];
     if (threadIdx.x == 0) s_m = mtab[q];
     __syncthreads();
     T A[O * O], B[O * O];

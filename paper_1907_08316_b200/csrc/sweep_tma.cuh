@@ -131,7 +131,7 @@ sweep_x1_bulk_kernel(const T *__restrict__ in, T *__restrict__ out, int n, long 
         bulk_g2s(s_in, in + base, bytes, &bar);
     }
     const long q = g % qmod;
-    if (threadIdx.x < 2 * O * O) s_ab[threadIdx.x] = ab[(long)threadIdx.x * count + q];
+    for (int e = threadIdx.x; e < 2 * O * O; e += blockDim.x) s_ab[e] = ab[(long)e * count + q];
     if (threadIdx.x == 32) s_m = mtab[q];
     __syncthreads();
     T A[O * O], B[O * O];

@@ -20,7 +20,7 @@ def _coords(oracle, cfg):
 
 
 def test_node_coords_match_oracle_to_one_ulp(oracle):
-    for o in (1, 2, 3, 4):
+    for o in (1, 2, 3, 4, 5, 6):
         cfg = W.Config("c", 1, 1, (7, 5), o, (0.0, -6.0), (4 * np.pi, 6.0))
         s = make_solver(cfg, "f64")
         for d in range(2):
@@ -194,3 +194,13 @@ def test_mixed_dimension_steps(oracle, shape, dtype):
     got, ref, tg, tr = _run_config(oracle, cfg, dtype, cfg.steps)
     assert rel_err(got, ref) <= TOL[dtype]
     _check_traces(tg, tr, max(TOL[dtype], 1e-11))
+
+
+@pytest.mark.parametrize("o", [4, 5, 6])
+def test_high_order_2p2_steps(oracle, o):
+    """NEXT-3: the orders of the paper's performance study (o = 4, 6) in a 2+2 D Landau step."""
+    cfg = W.Config("ho", 2, 2, (6, 5, 8, 7), o, (0.0, 0.0, -6.0, -6.0), (4 * np.pi, 4 * np.pi, 6.0, 6.0),
+                   dt=0.1, steps=3, kind="landau", eps=0.05, k=0.5)
+    got, ref, tg, tr = _run_config(oracle, cfg, "f64", cfg.steps)
+    assert rel_err(got, ref) <= TOL["f64"]
+    _check_traces(tg, tr, 1e-11)

@@ -36,7 +36,7 @@ def _sweep_case(oracle, cfg, dtype, dim, kind, seed):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("o", [1, 2, 3, 4])
+@pytest.mark.parametrize("o", [1, 2, 3, 4, 5, 6])
 @pytest.mark.parametrize("kind", ["small", "wide", "integer", "huge"])
 def test_sweep_1p1(oracle, o, dtype, kind):
     cfg = W.Config("t11", 1, 1, (37, 29), o, (0.0, -3.0), (5.0, 3.0))
@@ -230,3 +230,27 @@ def test_step_fused_equals_step_unfused_bitwise(monkeypatch):
         s.close()
     assert np.array_equal(outs[0][0], outs[1][0])
     assert outs[0][1] < outs[1][1]             # the fused step really launches fewer sweeps
+
+
+@pytest.mark.parametrize("o", [1, 2, 3, 4, 5, 6])
+def test_ab_tables_are_rounded_once(oracle, o):
+    """Unit impulses pick out single entries of A(theta) and B(theta): the library's table
+    (binary128 coefficients + double-double Horner) against the oracle's (long-double quadrature),
+    both meant to be the exact value rounded once (D:O7) -- they may differ by one ulp at most."""
+    n, nv = 5, 40
+    cfg = W.Config("ab", 1, 1, (n, nv), o, (0.0, 0.0), (1.0, 1.0))
+    rng = np.random.default_rng(o)
+    theta = rng.uniform(0.0, 1.0, cfg.N[1])
+    theta[:3] = (0.0, 0.5, 1.0 - 2.0 ** -40)
+    f0 = np.zeros((cfg.N[1], cfg.N[0]))
+    for q in range(cfg.N[1]):
+        f0[q, 2 * o + (q % o)] = 1.0                  # impulse in cell 2, local node q % o
+    f0 = f0.reshape(-1)
+    s = make_solver(cfg, "f64")
+    s.set_initial(f0)
+    s.translate(0, -theta)                            # sigma = -theta  ->  m = 0, theta as given
+    got = s.get_f()
+    s.close()
+    ref = oracle.translate(f0.copy(), cfg.N, o, 0, -theta, [1])
+    assert np.max(np.abs(got - ref)) <= 2.3e-16 * max(1.0, np.max(np.abs(ref)))
+    assert np.mean(got != ref) < 0.02                 # and almost always the very same double

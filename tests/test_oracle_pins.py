@@ -158,3 +158,13 @@ def test_assemble_rejects_theta_outside_unit_interval(oracle):
         oracle.assemble_AB(2, 1.0)
     with pytest.raises(ValueError):
         oracle.assemble_AB(2, -0.1)
+
+
+def test_R3_shift_split_never_returns_theta_one(oracle):
+    """delta = -sigma a hair below an integer: fl(delta - floor(delta)) rounds to 1.0; R3 makes it
+    the next integer shift with theta = 0 (the translation is continuous across integers)."""
+    for s, m_exp in ((1e-20, 0), (1.0 + 1e-17, -1), (-3.0 + 1e-18, 3)):
+        m, th = oracle.shift_split(s)
+        assert 0.0 <= th < 1.0 and (m, th) == (m_exp, 0.0)
+    assert oracle.shift_split(-1e-20) == (0, 1e-20)
+    assert oracle.shift_split(-0.25) == (0, 0.25) and oracle.shift_split(0.25) == (-1, 0.75)
