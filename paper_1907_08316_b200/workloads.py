@@ -80,6 +80,12 @@ CONFIG4 = Config("config4-sweep-2+2", 2, 2, (128, 128, 64, 64), 3, (0.0, 0.0, 0.
 CONFIG5 = Config("config5-landau-3+3", 3, 3, (20,) * 6, 2, (0.0, 0.0, 0.0, -6.0, -6.0, -6.0),
                  (4 * _PI,) * 3 + (6.0,) * 3, dt=0.1, steps=5, kind="landau", eps=0.01, k=0.5)
 
+# S:8(f) NEXT-2 -- the paper's validation run (section 8, eq. (2)): 2+2 D two-stream instability,
+# 60^4 cells, o = 4, t <= 100.  The paper does not print its time step: dt = 0.1 is this build's choice.
+PAPER_TWOSTREAM = Config("paper-twostream-2+2", 2, 2, (60, 60, 60, 60), 4, (0.0, 0.0, -6.0, -6.0),
+                         (10 * _PI, 10 * _PI, 6.0, 6.0), dt=0.1, steps=1000, kind="twostream2",
+                         eps=1e-3, k=0.2, extra={"v0": 2.4})
+
 CONFIGS = {c.name.split("-")[0]: c for c in (CONFIG1, CONFIG2, CONFIG3, CONFIG4, CONFIG5)}
 
 
@@ -113,6 +119,14 @@ def initial_factors(cfg, coords):
         gx = 1.0 + cfg.eps * _flat_sum([np.cos(cfg.k * np.asarray(x)) for x in xs])
         gv = _flat_outer([np.asarray(v) ** 2 * np.exp(-0.5 * np.asarray(v) ** 2) / np.sqrt(2.0 * np.pi)
                           for v in vs])
+    elif cfg.kind == "twostream2":
+        # the paper's own validation state, eq. (2):
+        # (1 + eps sum_a cos(k x_a)) * prod_a (exp(-(v_a-v0)^2/2) + exp(-(v_a+v0)^2/2)) / (2 sqrt(2 pi))
+        # (= 1/(8 pi) times the two brackets for d_v = 2)
+        v0 = float(cfg.extra["v0"])
+        gx = 1.0 + cfg.eps * _flat_sum([np.cos(cfg.k * np.asarray(x)) for x in xs])
+        gv = _flat_outer([(np.exp(-0.5 * (np.asarray(v) - v0) ** 2) + np.exp(-0.5 * (np.asarray(v) + v0) ** 2))
+                          / (2.0 * np.sqrt(2.0 * np.pi)) for v in vs])
     else:
         raise ValueError("config kind %r has no analytic initial state" % cfg.kind)
     return gx, gv

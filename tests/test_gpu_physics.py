@@ -204,3 +204,25 @@ def test_high_order_2p2_steps(oracle, o):
     got, ref, tg, tr = _run_config(oracle, cfg, "f64", cfg.steps)
     assert rel_err(got, ref) <= TOL["f64"]
     _check_traces(tg, tr, 1e-11)
+
+
+# ---------------------------------------------------------------- NEXT-2: the paper's validation run (eq. (2))
+
+def test_paper_twostream_parity_small(oracle):
+    cfg = W.PAPER_TWOSTREAM.scaled((8, 8, 10, 10), steps=5)
+    got, ref, tg, tr = _run_config(oracle, cfg, "f64", cfg.steps)
+    assert rel_err(got, ref) <= TOL["f64"]
+    _check_traces(tg, tr, 1e-11)
+
+
+def test_paper_twostream_fp32_vs_fp64_reduced():
+    """Reduced twin (20^4 cells, o = 4) of the paper's run to t = 40: the instability develops
+    (electric energy grows by orders of magnitude) and single vs double precision stay within the
+    paper's 'below 2e-4' in f, E and electric energy; mass is conserved."""
+    from paper_1907_08316_b200.examples.two_stream_2p2 import run
+    out, trace = run(cells=20, t_end=40.0, dt=0.1, sample_every=20)
+    assert out["ee_growth"] > 1e3
+    assert out["max_df_inf"] < 2e-4 and out["max_dE_inf"] < 2e-4
+    assert out["max_rel_ee_diff_vs_trace_max"] < 2e-4
+    assert out["mass_drift64"] < 1e-12 and out["mass_drift32"] < 1e-5
+    assert out["energy_drift64"] < 1e-2

@@ -74,3 +74,21 @@ def test_initial_state_is_separable_outer_product():
         * np.exp(-0.5 * (coords[2][p[1]] ** 2 + coords[3][p[0]] ** 2)) / (2 * np.pi)
     assert abs(F[p] - val) < 1e-16
     assert W.initial_state(cfg, coords, np.float32).dtype == np.float32
+
+
+def test_paper_twostream_state_eq2():
+    # PAPER.md eq. (2): f_eq integrates to 1 over v (each bracket to 2 sqrt(2 pi)), peaks near +-v0
+    cfg = W.PAPER_TWOSTREAM
+    assert cfg.order == 4 and cfg.cells == (60,) * 4 and cfg.extra["v0"] == 2.4
+    v = np.linspace(-12, 12, 4801)
+    x = np.array([0.0])
+    gx, gv = W.initial_factors(cfg, [x, x, v, v])
+    dv = v[1] - v[0]
+    assert abs(gv.sum() * dv * dv - 1.0) < 1e-9
+    assert abs(gx[0] - (1 + 2e-3)) < 1e-15
+    F = gv.reshape(v.size, v.size)
+    i, j = np.unravel_index(np.argmax(F), F.shape)
+    assert abs(abs(v[i]) - 2.4) < 0.02 and abs(abs(v[j]) - 2.4) < 0.02
+    # value at (v1, v2) = (v0, v0): (1 + e^{-2 v0^2})^2 / (8 pi)
+    k = np.argmin(np.abs(v - 2.4))
+    assert abs(F[k, k] - (1 + np.exp(-2 * 2.4 ** 2)) ** 2 / (8 * np.pi)) < 1e-12
