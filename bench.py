@@ -27,6 +27,13 @@ sys.path.insert(0, ROOT)
 
 from paper_1907_08316_b200 import workloads as W  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the sweep kernel of each direction, from one
+# ncu capture of this very command at full size (profiles/traffic_fullsize_r1c.md); None where not captured.
+TRAFFIC_BYTES = {
+    ("config4-sweep-2+2", "f64"): {0: 43.489e9 + 43.437e9, 1: 43.830e9 + 43.439e9,
+                                   2: 43.703e9 + 43.428e9, 3: 43.698e9 + 43.428e9},
+}
+
 METRIC = "achieved_hbm_gbs_per_translation_sweep"
 UNIT = "GB/s"
 
@@ -362,7 +369,9 @@ def run_ours(args):
     dim_avg = {d: float(np.mean(v)) for d, v in per_dim.items()}
     dom = max(dim_avg, key=dim_avg.get)
     roofline = {"bound": "hbm", "achieved": sweep_bytes / dim_avg[dom] / 1e6, "peak": peak, "unit": "GB/s",
-                "frac": sweep_bytes / dim_avg[dom] / 1e6 / peak, "traffic": None,
+                "frac": sweep_bytes / dim_avg[dom] / 1e6 / peak,
+                "traffic": TRAFFIC_BYTES.get((cfg.name, dtype), {}).get(dom),
+                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/traffic_fullsize_r1c.md",
                 "kernel": "translation sweep along dim %d (slowest direction)" % dom,
                 "algorithmic_bytes_per_launch": sweep_bytes, "peak_source": peak_src,
                 "per_direction_gbs": {"dim%d" % d: sweep_bytes / t / 1e6 for d, t in dim_avg.items()},
