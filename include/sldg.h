@@ -114,6 +114,14 @@ int sldg_advect_pair(sldg_ctx *ctx, int dim1, int dim2, double dt);
 int sldg_translate_pair_dev(sldg_ctx *ctx, int dim1, const double *shift1_device, size_t count1,
                             int dim2, const double *shift2_device, size_t count2);
 
+/* Three consecutive sweeps (dim1 < dim2 < dim3, all x- or all v-dimensions: the 3+3 D step) in one
+ * pass over f; identical, bit for bit, to the three single sweeps.  The fused kernel exists for
+ * order <= 2; above that the call runs a fused pair followed by a single sweep (same result). */
+int sldg_advect_triple(sldg_ctx *ctx, int dim1, int dim2, int dim3, double dt);
+int sldg_translate_triple_dev(sldg_ctx *ctx, int dim1, const double *shift1_device, size_t count1,
+                              int dim2, const double *shift2_device, size_t count2,
+                              int dim3, const double *shift3_device, size_t count3);
+
 /* rho[X] = -sum_v W_v f[v][x] (fp64 accumulation for both dtypes) into the
  * context and, if rho_device_or_null != NULL, also to that device array. */
 int sldg_compute_rho(sldg_ctx *ctx, double *rho_device_or_null);

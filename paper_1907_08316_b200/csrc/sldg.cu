@@ -54,12 +54,12 @@ struct sldg_ctx {
         double tau = 0.0;
         bool valid = false;            // m/ab hold the assembled table for `tau`
     };
-    Tab gen[2], xt[3];
+    Tab gen[3], xt[3];
     // the table set(s) the next sweep launch reads: aliases into gen[] / xt[]
-    double *d_sigma = nullptr, *d_sigma2 = nullptr;
-    int *d_m = nullptr, *d_m2 = nullptr;
-    void *d_ab = nullptr, *d_ab2 = nullptr;
-    bool skip_asm1 = false, skip_asm2 = false;
+    double *d_sigma = nullptr, *d_sigma2 = nullptr, *d_sigma3 = nullptr;
+    int *d_m = nullptr, *d_m2 = nullptr, *d_m3 = nullptr;
+    void *d_ab = nullptr, *d_ab2 = nullptr, *d_ab3 = nullptr;
+    bool skip_asm1 = false, skip_asm2 = false, skip_asm3 = false;
     double *d_Wv = nullptr, *d_Wx = nullptr;      // quadrature weights over v-nodes / x-nodes
     double *d_va = nullptr, *d_v2 = nullptr;      // per v-node: coordinates v_a [dv][V] and |v|^2 [V]
     double *d_rho = nullptr, *d_s2 = nullptr, *d_E = nullptr;   // [X], [X], [dx][X]
@@ -587,10 +587,69 @@ int run_pair(sldg_ctx *c, int k1, int k2, long count1, long count2) {
     return fail(c, SLDG_ERR_UNSUPPORTED, "order %d not instantiated", c->o);
 }
 
+// ---- fused triple of sweeps (sweep_fused.cuh: sweep_triple_kernel), o <= 2 -------------------
+template <typename T, int O>
+int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long cnt3) {
+    const int n1 = c->cells[k1], n2 = c->cells[k2], n3 = c->cells[k3];
+    const T *in = (const T *)c->buf[c->cur];
+    T *out = (T *)c->buf[c->cur ^ 1];
+    int block = 128;
+    size_t sh = (size_t)2 * O * O * 2 * O * 2 * sizeof(double);
+    const bool skip[3] = {c->skip_asm1, c->skip_asm2, c->skip_asm3};
+    double *sg[3] = {c->d_sigma, c->d_sigma2, c->d_sigma3};
+    int *mm[3] = {c->d_m, c->d_m2, c->d_m3};
+    void *ab[3] = {c->d_ab, c->d_ab2, c->d_ab3};
+    const long cnt[3] = {cnt1, cnt2, cnt3};
+    const int nn[3] = {n1, n2, n3};
+    for (int i = 0; i < 3; ++i)
+        if (!skip[i]) {
+            assemble_ab_kernel<T><<<(unsigned)cdiv(cnt[i], block), block, sh, c->stream>>>(
+                sg[i], cnt[i], O, nn[i], c->d_coef, mm[i], (T *)ab[i]);
+            LAUNCH_CHECK(c);
+        }
+    long inner1 = 1, mid12 = 1, mid23 = 1, outer3 = 1;
+    for (int d = 0; d < k1; ++d) inner1 *= c->N[d];
+    for (int d = k1 + 1; d < k2; ++d) mid12 *= c->N[d];
+    for (int d = k2 + 1; d < k3; ++d) mid23 *= c->N[d];
+    for (int d = k3 + 1; d < c->D; ++d) outer3 *= c->N[d];
+    long qd[3], qm[3];
+    const int ks[3] = {k1, k2, k3};
+    for (int i = 0; i < 3; ++i) {
+        if (ks[i] < c->dx) {
+            qd[i] = 1;
+            for (int d = 0; d < c->dx + ks[i]; ++d) qd[i] *= c->N[d];
+            qm[i] = c->N[c->dx + ks[i]];
+        } else { qd[i] = 1; qm[i] = c->X; }
+    }
+    int chunk = 32;
+    while (inner1 % chunk) chunk /= 2;
+    long threads = inner1 * n1 * mid12 * n2 * mid23 * outer3;
+    sweep_triple_kernel<T, O><<<(unsigned)cdiv(threads, 128), 128, 0, c->stream>>>(
+        in, out, inner1, n1, mid12, n2, mid23, n3, outer3, chunk,
+        mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2, qd[1], qm[1],
+        mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+    LAUNCH_CHECK(c);
+    c->cur ^= 1;
+    c->have_rho = false;
+    return SLDG_OK;
+}
+
+int run_triple(sldg_ctx *c, int k1, int k2, int k3, long c1, long c2, long c3) {
+    if (c->dtype == SLDG_F64) {
+        if (c->o == 1) return run_triple_t<double, 1>(c, k1, k2, k3, c1, c2, c3);
+        if (c->o == 2) return run_triple_t<double, 2>(c, k1, k2, k3, c1, c2, c3);
+    } else {
+        if (c->o == 1) return run_triple_t<float, 1>(c, k1, k2, k3, c1, c2, c3);
+        if (c->o == 2) return run_triple_t<float, 2>(c, k1, k2, k3, c1, c2, c3);
+    }
+    return fail(c, SLDG_ERR_UNSUPPORTED, "fused triple is instantiated for order <= 2 (got %d)", c->o);
+}
+
 // point table slot 1 or 2 at a storage set; `assembled` = its m/ab are already valid
 void use_tab(sldg_ctx *c, int slot, sldg_ctx::Tab &t, bool assembled) {
     if (slot == 1) { c->d_sigma = t.sigma; c->d_m = t.m; c->d_ab = t.ab; c->skip_asm1 = assembled; }
-    else { c->d_sigma2 = t.sigma; c->d_m2 = t.m; c->d_ab2 = t.ab; c->skip_asm2 = assembled; }
+    else if (slot == 2) { c->d_sigma2 = t.sigma; c->d_m2 = t.m; c->d_ab2 = t.ab; c->skip_asm2 = assembled; }
+    else { c->d_sigma3 = t.sigma; c->d_m3 = t.m; c->d_ab3 = t.ab; c->skip_asm3 = assembled; }
 }
 
 long sweep_count(const sldg_ctx *c, int dim) { return dim < c->dx ? c->N[c->dx + dim] : c->X; }
@@ -821,10 +880,48 @@ extern "C" int sldg_set_E(sldg_ctx *c, const double *E, int is_device) {
     return SLDG_OK;
 }
 
+extern "C" int sldg_advect_triple(sldg_ctx *c, int dim1, int dim2, int dim3, double dt) {
+    if (!c) return SLDG_ERR_ARG;
+    if (!pair_ok(c, dim1, dim2) || !pair_ok(c, dim2, dim3) || !pair_ok(c, dim1, dim3))
+        return fail(c, SLDG_ERR_ARG, "sldg_advect_triple: need dim1 < dim2 < dim3, all x- or all v-dimensions");
+    if (c->o > 2) {                      // the triple kernel is instantiated for o <= 2 (registers)
+        int r = sldg_advect_pair(c, dim1, dim2, dt);
+        return r ? r : sldg_advect(c, dim3, dt);
+    }
+    int rc;
+    if ((rc = physics_tab(c, 1, dim1, dt))) return rc;
+    if ((rc = physics_tab(c, 2, dim2, dt))) return rc;
+    if ((rc = physics_tab(c, 3, dim3, dt))) return rc;
+    return run_triple(c, dim1, dim2, dim3, sweep_count(c, dim1), sweep_count(c, dim2), sweep_count(c, dim3));
+}
+
+extern "C" int sldg_translate_triple_dev(sldg_ctx *c, int dim1, const double *shift1, size_t count1, int dim2,
+                                         const double *shift2, size_t count2, int dim3, const double *shift3,
+                                         size_t count3) {
+    if (!c || !shift1 || !shift2 || !shift3) return SLDG_ERR_ARG;
+    if (!pair_ok(c, dim1, dim2) || !pair_ok(c, dim2, dim3) || !pair_ok(c, dim1, dim3))
+        return fail(c, SLDG_ERR_ARG, "sldg_translate_triple_dev: need dim1 < dim2 < dim3, all x- or all v-dimensions");
+    if ((long)count1 != sweep_count(c, dim1) || (long)count2 != sweep_count(c, dim2) ||
+        (long)count3 != sweep_count(c, dim3))
+        return fail(c, SLDG_ERR_ARG, "sldg_translate_triple_dev: wrong shift counts");
+    if (c->o > 2) {
+        int r = sldg_translate_pair_dev(c, dim1, shift1, count1, dim2, shift2, count2);
+        return r ? r : sldg_translate_dev(c, dim3, shift3, count3);
+    }
+    use_tab(c, 1, c->gen[0], false);
+    use_tab(c, 2, c->gen[1], false);
+    use_tab(c, 3, c->gen[2], false);
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift1, count1 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma2, shift2, count2 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma3, shift3, count3 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    return run_triple(c, dim1, dim2, dim3, (long)count1, (long)count2, (long)count3);
+}
+
 namespace {
 // sweeps along dimensions base .. base+cnt-1 with increment tau, fusing the first two when allowed
 int advect_group(sldg_ctx *c, int base, int cnt, double tau) {
     int rc, a = 0;
+    if (c->use_fuse && cnt == 3 && c->o <= 2) return sldg_advect_triple(c, base, base + 1, base + 2, tau);
     if (c->use_fuse && cnt >= 2) {
         if ((rc = sldg_advect_pair(c, base, base + 1, tau))) return rc;
         a = 2;

@@ -137,3 +137,131 @@ sweep_pair_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, in
 }
 
 }  // namespace sldg
+
+namespace sldg {
+
+// ------------------------------------------------------------------------------------------
+// THREE consecutive sweeps (k1 < k2 < k3, all x- or all v-dimensions: the 3+3 D step) in one pass.
+// Same idea one level up: a thread owns one k1-cell x one k2-cell (O x O nodes) at fixed other
+// indices and walks the k3 line.  For every new k3-cell and each of its O rows it loads the raw
+// values of the 2 x 2 source cells (4 O^2 values), applies the k1 rule (-> 2 O^2 values), then
+// the k2 rule (-> the O^2 values of ITS OWN cell pair), which form its private sliding window
+// along k3; the k3 rule emits O^3 outputs per k3-cell.  Bit-identical to the three sweeps.
+// Each raw value is needed by 4 threads (neighbours in c1, c2): L1/L2 hits, DRAM sees one read
+// and one write of f for three sweeps.  Instantiated for O <= 2 (4 O^3 raw values per cell).
+// ------------------------------------------------------------------------------------------
+template <typename T, int O>
+__global__ void __launch_bounds__(128)
+sweep_triple_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, int n1, long mid12, int n2,
+                    long mid23, int n3, long outer3, int chunk,
+                    const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
+                    const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2,
+                    const int *__restrict__ mtab3, const T *__restrict__ ab3, long count3, long qdiv3, long qmod3) {
+    long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long il = t % chunk; t /= chunk;
+    const int c1 = (int)(t % n1); t /= n1;
+    const long ih = t % (inner1 / chunk); t /= (inner1 / chunk);
+    const long ii = ih * chunk + il;
+    const long m12 = t % mid12; t /= mid12;
+    const int c2 = (int)(t % n2); t /= n2;
+    const long m23 = t % mid23;
+    const long oo3 = t / mid23;
+    if (oo3 >= outer3) return;
+
+    const long s1 = inner1;
+    const long s2 = mid12 * (long)n1 * O * s1;
+    const long s3 = mid23 * (long)n2 * O * s2;
+    const long base = oo3 * (long)n3 * O * s3 + m23 * (long)n2 * O * s2 + m12 * (long)n1 * O * s1 + ii;
+    const long own = (long)c1 * O * s1 + (long)c2 * O * s2;
+    const long lin0 = base + own;
+    const long q1 = (lin0 / qdiv1) % qmod1, q2 = (lin0 / qdiv2) % qmod2, q3 = (lin0 / qdiv3) % qmod3;
+
+    T A1[O * O], B1[O * O], A2[O * O], B2[O * O], A3[O * O], B3[O * O];
+#pragma unroll
+    for (int e = 0; e < O * O; ++e) {
+        A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1];
+        A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
+        A3[e] = ab3[(long)e * count3 + q3]; B3[e] = ab3[(long)(O * O + e) * count3 + q3];
+    }
+    const int m1 = mtab1[q1], m2 = mtab2[q2], m3 = mtab3[q3];
+    int sa1 = c1 + m1; if (sa1 >= n1) sa1 -= n1;
+    int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
+    int sa2 = c2 + m2; if (sa2 >= n2) sa2 -= n2;
+    int sb2 = sa2 + 1; if (sb2 == n2) sb2 = 0;
+    // offsets of the 2 x 2 source cells (k2 cell, k1 cell) relative to `base`
+    const long off[2][2] = {{(long)sa2 * O * s2 + (long)sa1 * O * s1, (long)sa2 * O * s2 + (long)sb1 * O * s1},
+                            {(long)sb2 * O * s2 + (long)sa1 * O * s1, (long)sb2 * O * s2 + (long)sb1 * O * s1}};
+
+    // raw[l3][cell2][l2][cell1][l1]
+    auto load_raw = [&](int cell3, T (&r)[O][2][O][2][O]) {
+#pragma unroll
+        for (int l3 = 0; l3 < O; ++l3) {
+            const T *row = in + base + ((long)cell3 * O + l3) * s3;
+#pragma unroll
+            for (int e2 = 0; e2 < 2; ++e2)
+#pragma unroll
+                for (int l2 = 0; l2 < O; ++l2)
+#pragma unroll
+                    for (int e1 = 0; e1 < 2; ++e1)
+#pragma unroll
+                        for (int l1 = 0; l1 < O; ++l1) r[l3][e2][l2][e1][l1] = row[off[e2][e1] + l2 * s2 + l1 * s1];
+        }
+    };
+    // k1 rule then k2 rule: w[l3][j2][j1] = the (k1,k2)-swept values of this thread's own cell pair
+    auto k12_rule = [&](const T (&r)[O][2][O][2][O], T (&w)[O][O][O]) {
+#pragma unroll
+        for (int l3 = 0; l3 < O; ++l3) {
+            T tk[2][O][O];                                   // k1-swept: [cell2][l2][j1]
+#pragma unroll
+            for (int e2 = 0; e2 < 2; ++e2)
+#pragma unroll
+                for (int l2 = 0; l2 < O; ++l2)
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) tk[e2][l2][j1] = chain<T, O>(A1, B1, j1, r[l3][e2][l2][0], r[l3][e2][l2][1]);
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a0[O], a1[O];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) { a0[l] = tk[0][l][j1]; a1[l] = tk[1][l][j1]; }
+                    w[l3][j2][j1] = chain<T, O>(A2, B2, j2, a0, a1);
+                }
+        }
+    };
+
+    int is3 = m3;                                            // source k3-cell of output cell 0
+    T raw[O][2][O][2][O], w0[O][O][O], w1[O][O][O];
+    load_raw(is3, raw);
+    k12_rule(raw, w0);
+    if (++is3 == n3) is3 = 0;
+    load_raw(is3, raw);
+    T *dst = out + lin0;
+    for (int i3 = 0; i3 < n3; ++i3) {
+        k12_rule(raw, w1);
+        if (i3 + 1 < n3) {                                   // next cell's loads fly during the arithmetic below
+            if (++is3 == n3) is3 = 0;
+            load_raw(is3, raw);
+        }
+#pragma unroll
+        for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a0[O], a1[O];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) { a0[l] = w0[l][j2][j1]; a1[l] = w1[l][j2][j1]; }
+                    dst[(long)j3 * s3 + (long)j2 * s2 + j1 * s1] = chain<T, O>(A3, B3, j3, a0, a1);
+                }
+#pragma unroll
+        for (int l = 0; l < O; ++l)
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) w0[l][j2][j1] = w1[l][j2][j1];
+        dst += (long)O * s3;
+    }
+}
+
+}  // namespace sldg

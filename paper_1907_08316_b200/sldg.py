@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libsldg.so")
 EXPORTS = [
     "sldg_create", "sldg_destroy", "sldg_last_error", "sldg_num_dofs", "sldg_num_x",
     "sldg_node_coords", "sldg_set_initial", "sldg_get_f", "sldg_current", "sldg_fill_uniform",
-    "sldg_translate", "sldg_translate_dev", "sldg_advect", "sldg_advect_pair", "sldg_translate_pair_dev", "sldg_compute_rho", "sldg_poisson_E",
+    "sldg_translate", "sldg_translate_dev", "sldg_advect", "sldg_advect_pair", "sldg_translate_pair_dev", "sldg_advect_triple", "sldg_translate_triple_dev", "sldg_compute_rho", "sldg_poisson_E",
     "sldg_set_E", "sldg_step", "sldg_diagnostics", "sldg_moments", "sldg_launch_count",
 ]
 
@@ -48,6 +48,8 @@ def _load():
     lib.sldg_advect.argtypes = [vp, C.c_int, C.c_double]
     lib.sldg_advect_pair.argtypes = [vp, C.c_int, C.c_int, C.c_double]
     lib.sldg_translate_pair_dev.argtypes = [vp, C.c_int, vp, C.c_size_t, C.c_int, vp, C.c_size_t]
+    lib.sldg_advect_triple.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_double]
+    lib.sldg_translate_triple_dev.argtypes = [vp] + [C.c_int, vp, C.c_size_t] * 3
     lib.sldg_compute_rho.argtypes = [vp, vp]
     lib.sldg_poisson_E.argtypes = [vp, vp]
     lib.sldg_set_E.argtypes = [vp, vp, C.c_int]
@@ -173,6 +175,15 @@ class Sldg:
             assert t.is_cuda and t.dtype == self.torch.float64 and t.is_contiguous()
         self._chk(_lib.sldg_translate_pair_dev(self.h, dim1, shift1.data_ptr(), shift1.numel(),
                                                dim2, shift2.data_ptr(), shift2.numel()), "translate_pair_dev")
+
+    def advect_triple(self, d1, d2, d3, dt):
+        self._chk(_lib.sldg_advect_triple(self.h, d1, d2, d3, float(dt)), "advect_triple")
+
+    def translate_triple(self, d1, s1, d2, s2, d3, s3):
+        for t in (s1, s2, s3):
+            assert t.is_cuda and t.dtype == self.torch.float64 and t.is_contiguous()
+        self._chk(_lib.sldg_translate_triple_dev(self.h, d1, s1.data_ptr(), s1.numel(), d2, s2.data_ptr(),
+                                                 s2.numel(), d3, s3.data_ptr(), s3.numel()), "translate_triple_dev")
 
     def compute_rho(self, out=True):
         """rho into the context; with out=True also returned as a new device tensor."""

@@ -254,3 +254,49 @@ def test_ab_tables_are_rounded_once(oracle, o):
     ref = oracle.translate(f0.copy(), cfg.N, o, 0, -theta, [1])
     assert np.max(np.abs(got - ref)) <= 2.3e-16 * max(1.0, np.max(np.abs(ref)))
     assert np.mean(got != ref) < 0.02                 # and almost always the very same double
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("o", [1, 2, 3])
+def test_fused_triple_is_bitwise_the_three_sweeps_3p3(oracle, o, dtype):
+    """x_1,x_2,x_3 and v_1,v_2,v_3 in one pass each (o <= 2: the triple kernel; o = 3: pair + single)."""
+    import torch
+    cfg = W.Config("t33", 3, 3, (5, 4, 6, 4, 5, 3), o, (0.0,) * 6, (5.0, 4.0, 6.0, 4.0, 5.0, 3.0))
+    rng = np.random.default_rng(31 + o)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
+    for ks in ((0, 1, 2), (3, 4, 5)):
+        sig = [rng.uniform(-2.5, 2.5, cfg.N[cfg.dx + k] if k < cfg.dx else cfg.X) for k in ks]
+        a = make_solver(cfg, dtype)
+        a.set_initial(f0)
+        a.translate_triple(ks[0], torch.from_numpy(sig[0]).cuda(), ks[1], torch.from_numpy(sig[1]).cuda(),
+                           ks[2], torch.from_numpy(sig[2]).cuda())
+        fused = a.get_f()
+        a.close()
+        b = make_solver(cfg, dtype)
+        b.set_initial(f0)
+        for k, s_ in zip(ks, sig):
+            b.translate(k, s_)
+        seq = b.get_f()
+        b.close()
+        assert np.array_equal(fused, seq), ks
+        ref = f0.copy()
+        for k, s_ in zip(ks, sig):
+            oracle.translate(ref, cfg.N, cfg.order, k, s_, dep_of(cfg.dx, k))
+        assert rel_err(fused, ref) <= TOL[dtype], ks
+
+
+def test_step_3p3_fused_equals_unfused_bitwise(monkeypatch):
+    cfg = W.CONFIG5.scaled((6, 5, 4, 6, 4, 5))
+    outs = []
+    for flag in ("0", "1"):
+        monkeypatch.setenv("SLDG_NO_FUSE", flag)
+        s = make_solver(cfg, "f64")
+        coords = [s.node_coords(d) for d in range(6)]
+        s.set_initial(W.initial_state(cfg, coords))
+        l0 = s.launch_count()
+        for _ in range(2):
+            s.step(cfg.dt)
+        outs.append((s.get_f(), s.launch_count() - l0))
+        s.close()
+    assert np.array_equal(outs[0][0], outs[1][0])
+    assert outs[0][1] < outs[1][1]
