@@ -157,13 +157,16 @@ sweep_triple_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, 
                     const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
                     const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2,
                     const int *__restrict__ mtab3, const T *__restrict__ ab3, long count3, long qdiv3, long qmod3) {
+    // thread order: lanes along inner1 (chunk), then c1, then c2: the 4 threads that read one raw
+    // value (owners of (c1, c2), (c1-1, c2), (c1, c2-1), (c1-1, c2-1)) are at most chunk*n1 threads
+    // apart, so the repeats are L1/L2 hits (with c2 further out, the v-triple re-read f from HBM).
     long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
     const long il = t % chunk; t /= chunk;
     const int c1 = (int)(t % n1); t /= n1;
+    const int c2 = (int)(t % n2); t /= n2;
     const long ih = t % (inner1 / chunk); t /= (inner1 / chunk);
     const long ii = ih * chunk + il;
     const long m12 = t % mid12; t /= mid12;
-    const int c2 = (int)(t % n2); t /= n2;
     const long m23 = t % mid23;
     const long oo3 = t / mid23;
     if (oo3 >= outer3) return;
