@@ -565,9 +565,11 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
     long threads = lines * nseg;
     int chunk = 32;
     while (inner1 % chunk) chunk /= 2;
-    sweep_pair_kernel<T, O><<<(unsigned)cdiv(threads, 128), 128, 0, c->stream>>>(
-        in, out, inner1, n1, midN, n2, outer2, nseg, cps, chunk, c->d_m, (const T *)c->d_ab, count1, qd1, qm1,
-        c->d_m2, (const T *)c->d_ab2, count2, qd2, qm2);
+    // (the vectorised-cell variant VEC1 helps the triple kernel but measured slower for the pair
+    //  kernel at config 3: 0.906 vs 0.704 ms, so the pair always uses scalar accesses)
+    sweep_pair_kernel<T, O, false><<<(unsigned)cdiv(threads, 128), 128, 0, c->stream>>>(
+            in, out, inner1, n1, midN, n2, outer2, nseg, cps, chunk, c->d_m, (const T *)c->d_ab, count1, qd1, qm1,
+            c->d_m2, (const T *)c->d_ab2, count2, qd2, qm2);
     LAUNCH_CHECK(c);
     c->cur ^= 1;
     c->have_rho = false;
@@ -624,10 +626,16 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
     int chunk = 32;
     while (inner1 % chunk) chunk /= 2;
     long threads = inner1 * n1 * mid12 * n2 * mid23 * outer3;
-    sweep_triple_kernel<T, O><<<(unsigned)cdiv(threads, 128), 128, 0, c->stream>>>(
-        in, out, inner1, n1, mid12, n2, mid23, n3, outer3, chunk,
-        mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2, qd[1], qm[1],
-        mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+    if (O % 2 == 0 && inner1 == 1)
+        sweep_triple_kernel<T, O, (O % 2 == 0)><<<(unsigned)cdiv(threads, 128), 128, 0, c->stream>>>(
+            in, out, inner1, n1, mid12, n2, mid23, n3, outer3, chunk,
+            mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2, qd[1], qm[1],
+            mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+    else
+        sweep_triple_kernel<T, O, false><<<(unsigned)cdiv(threads, 128), 128, 0, c->stream>>>(
+            in, out, inner1, n1, mid12, n2, mid23, n3, outer3, chunk,
+            mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2, qd[1], qm[1],
+            mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
     LAUNCH_CHECK(c);
     c->cur ^= 1;
     c->have_rho = false;

@@ -21,7 +21,10 @@
 
 namespace sldg {
 
-template <typename T, int O>
+// VEC1: k1 is the contiguous x_1 line (inner1 == 1) and O is even, so the O nodes of a cell are
+// read / written as 2-element vectors (16 B in fp64): half the load/store requests and L1
+// wavefronts (the x-fused kernels were bound by the LSU pipe: 87 % wavefront utilisation in ncu).
+template <typename T, int O, bool VEC1>
 __global__ void __launch_bounds__(128)
 sweep_pair_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, int n1, long midN, int n2,
                   long outer2, int nseg, int cps, int chunk,
@@ -73,10 +76,21 @@ sweep_pair_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, in
 #pragma unroll
         for (int l2 = 0; l2 < O; ++l2) {
             const long ro = ((long)cell2 * O + l2) * stride2;
+            if constexpr (VEC1) {
+                using V2 = Vec<T, 2>;
 #pragma unroll
-            for (int l = 0; l < O; ++l) {
-                r0[l2][l] = src0[ro + l * s1];
-                r1[l2][l] = src1[ro + l * s1];
+                for (int l = 0; l < O; l += 2) {
+                    V2 a = *reinterpret_cast<const V2 *>(src0 + ro + l);
+                    V2 b = *reinterpret_cast<const V2 *>(src1 + ro + l);
+                    r0[l2][l] = a.v[0]; r0[l2][l + 1] = a.v[1];
+                    r1[l2][l] = b.v[0]; r1[l2][l + 1] = b.v[1];
+                }
+            } else {
+#pragma unroll
+                for (int l = 0; l < O; ++l) {
+                    r0[l2][l] = src0[ro + l * s1];
+                    r1[l2][l] = src1[ro + l * s1];
+                }
             }
         }
     };
@@ -92,12 +106,24 @@ sweep_pair_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, in
     auto emit = [&](T *dst, const T (&w0)[O][O], const T (&w1)[O][O]) {
 #pragma unroll
         for (int j2 = 0; j2 < O; ++j2) {
+            T res[O];
 #pragma unroll
             for (int j1 = 0; j1 < O; ++j1) {
                 T a0[O], a1[O];
 #pragma unroll
                 for (int l = 0; l < O; ++l) { a0[l] = w0[l][j1]; a1[l] = w1[l][j1]; }
-                dst[(long)j2 * stride2 + j1 * s1] = chain<T, O>(A2, B2, j2, a0, a1);
+                res[j1] = chain<T, O>(A2, B2, j2, a0, a1);
+            }
+            if constexpr (VEC1) {
+                using V2 = Vec<T, 2>;
+#pragma unroll
+                for (int j1 = 0; j1 < O; j1 += 2) {
+                    V2 v; v.v[0] = res[j1]; v.v[1] = res[j1 + 1];
+                    *reinterpret_cast<V2 *>(dst + (long)j2 * stride2 + j1) = v;
+                }
+            } else {
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) dst[(long)j2 * stride2 + j1 * s1] = res[j1];
             }
         }
     };
@@ -150,7 +176,7 @@ namespace sldg {
 // Each raw value is needed by 4 threads (neighbours in c1, c2): L1/L2 hits, DRAM sees one read
 // and one write of f for three sweeps.  Instantiated for O <= 2 (4 O^3 raw values per cell).
 // ------------------------------------------------------------------------------------------
-template <typename T, int O>
+template <typename T, int O, bool VEC1>
 __global__ void __launch_bounds__(128)
 sweep_triple_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, int n1, long mid12, int n2,
                     long mid23, int n3, long outer3, int chunk,
@@ -205,9 +231,19 @@ sweep_triple_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, 
 #pragma unroll
                 for (int l2 = 0; l2 < O; ++l2)
 #pragma unroll
-                    for (int e1 = 0; e1 < 2; ++e1)
+                    for (int e1 = 0; e1 < 2; ++e1) {
+                        if constexpr (VEC1) {
+                            using V2 = Vec<T, 2>;
 #pragma unroll
-                        for (int l1 = 0; l1 < O; ++l1) r[l3][e2][l2][e1][l1] = row[off[e2][e1] + l2 * s2 + l1 * s1];
+                            for (int l1 = 0; l1 < O; l1 += 2) {
+                                V2 a = *reinterpret_cast<const V2 *>(row + off[e2][e1] + l2 * s2 + l1);
+                                r[l3][e2][l2][e1][l1] = a.v[0]; r[l3][e2][l2][e1][l1 + 1] = a.v[1];
+                            }
+                        } else {
+#pragma unroll
+                            for (int l1 = 0; l1 < O; ++l1) r[l3][e2][l2][e1][l1] = row[off[e2][e1] + l2 * s2 + l1 * s1];
+                        }
+                    }
         }
     };
     // k1 rule then k2 rule: w[l3][j2][j1] = the (k1,k2)-swept values of this thread's own cell pair
@@ -249,14 +285,27 @@ sweep_triple_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, 
 #pragma unroll
         for (int j3 = 0; j3 < O; ++j3)
 #pragma unroll
-            for (int j2 = 0; j2 < O; ++j2)
+            for (int j2 = 0; j2 < O; ++j2) {
+                T res[O];
 #pragma unroll
                 for (int j1 = 0; j1 < O; ++j1) {
                     T a0[O], a1[O];
 #pragma unroll
                     for (int l = 0; l < O; ++l) { a0[l] = w0[l][j2][j1]; a1[l] = w1[l][j2][j1]; }
-                    dst[(long)j3 * s3 + (long)j2 * s2 + j1 * s1] = chain<T, O>(A3, B3, j3, a0, a1);
+                    res[j1] = chain<T, O>(A3, B3, j3, a0, a1);
                 }
+                if constexpr (VEC1) {
+                    using V2 = Vec<T, 2>;
+#pragma unroll
+                    for (int j1 = 0; j1 < O; j1 += 2) {
+                        V2 v; v.v[0] = res[j1]; v.v[1] = res[j1 + 1];
+                        *reinterpret_cast<V2 *>(dst + (long)j3 * s3 + (long)j2 * s2 + j1) = v;
+                    }
+                } else {
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) dst[(long)j3 * s3 + (long)j2 * s2 + j1 * s1] = res[j1];
+                }
+            }
 #pragma unroll
         for (int l = 0; l < O; ++l)
 #pragma unroll
