@@ -112,6 +112,7 @@ class Sldg:
         if getattr(self, "h", None):
             _lib.sldg_destroy(self.h)
             self.h = None
+            self.buf = None          # release the two f buffers
 
     def __del__(self):
         try:

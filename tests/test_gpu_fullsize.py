@@ -140,3 +140,55 @@ def test_config3_full_size_one_step_against_full_oracle(oracle):
     torch.cuda.empty_cache()
     assert err <= TOL["f64"]
     assert abs(ee - eer) <= 1e-12 * eer and abs(m - mr) <= 1e-12 * mr and abs(l2 - l2r) <= 1e-12 * l2r
+
+
+def _fused_vs_single_fullsize(cfg, dtype, groups, shifts_of, gb):
+    """Fused pair / triple at full size against the same single sweeps, bit for bit (two solvers).
+    The single sweeps are the ones checked against the oracle by the sampled-line tests above."""
+    import torch
+    _need_gb(gb)
+    a = make_solver(cfg, dtype)
+    b = make_solver(cfg, dtype)
+    a.fill_uniform(W.SEED, W.TAG_F)
+    b.fill_uniform(W.SEED, W.TAG_F)
+    for ks in groups:
+        sh = [torch.from_numpy(np.ascontiguousarray(shifts_of(k))).cuda() for k in ks]
+        if len(ks) == 3:
+            a.translate_triple(ks[0], sh[0], ks[1], sh[1], ks[2], sh[2])
+        else:
+            a.translate_pair(ks[0], sh[0], ks[1], sh[1])
+        for k, s_ in zip(ks, sh):
+            b.translate(k, s_)
+        fa, fb = a.current(), b.current()
+        same = True
+        chunk = 1 << 28
+        for i in range(0, fa.numel(), chunk):
+            same = same and bool(torch.equal(fa[i:i + chunk], fb[i:i + chunk]))
+        assert same, ks
+    a.close()
+    b.close()
+    torch.cuda.empty_cache()
+
+
+def _smooth_shifts(cfg):
+    def shifts(dim):
+        cnt = cfg.N[cfg.dx + dim] if dim < cfg.dx else cfg.X
+        if dim < cfg.dx:
+            va = cfg.dx + dim
+            h = (cfg.hi[dim] - cfg.lo[dim]) / cfg.cells[dim]
+            return np.linspace(cfg.lo[va], cfg.hi[va], cnt) * 0.5 * cfg.dt / h
+        return 0.3 * np.sin(2 * np.pi * np.arange(cnt) / cfg.N[0] + 0.1 * dim)     # smooth in x like E
+    return shifts
+
+
+def test_config5_full_size_fused_triples_equal_single_sweeps():
+    _fused_vs_single_fullsize(W.CONFIG5, "f64", [(0, 1, 2), (3, 4, 5)], _smooth_shifts(W.CONFIG5), 140)
+
+
+def test_config4_fp32_full_size_fused_pairs_equal_single_sweeps():
+    cfg = W.CONFIG4
+    _fused_vs_single_fullsize(cfg, "f32", [(0, 1), (2, 3)], lambda d: W.config4_shifts(cfg, d), 95)
+
+
+def test_config3_full_size_fused_pairs_equal_single_sweeps():
+    _fused_vs_single_fullsize(W.CONFIG3, "f64", [(0, 1), (2, 3)], _smooth_shifts(W.CONFIG3), 10)
