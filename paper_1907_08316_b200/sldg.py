@@ -72,7 +72,7 @@ class Sldg:
     """One solver context.  Allocates the two f buffers as torch CUDA tensors (caller-owned
     memory in the sense of sldg.h) and forwards every call to the library."""
 
-    def __init__(self, dx, dv, cells, order, lo, hi, dtype="f64", device="cuda:0", stream=None):
+    def __init__(self, dx, dv, cells, order, lo, hi, dtype="f64", device="cuda:0", stream=None, buffers=None):
         import torch
         if not torch.cuda.is_available():
             raise SldgError("no CUDA device: the SLDG library has no CPU path")
@@ -89,7 +89,12 @@ class Sldg:
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        self.buf = [torch.empty(self.ndof, dtype=self.tdtype, device=self.device) for _ in range(2)]
+        if buffers is None:
+            self.buf = [torch.empty(self.ndof, dtype=self.tdtype, device=self.device) for _ in range(2)]
+        else:       # caller-owned device buffers (two contiguous CUDA tensors of N values each)
+            self.buf = list(buffers)
+            for b in self.buf:
+                assert b.is_cuda and b.dtype == self.tdtype and b.numel() == self.ndof and b.is_contiguous()
         cells_a = (C.c_int * D)(*self.cells)
         lo_a = (C.c_double * D)(*[float(x) for x in lo])
         hi_a = (C.c_double * D)(*[float(x) for x in hi])

@@ -300,3 +300,40 @@ def test_step_3p3_fused_equals_unfused_bitwise(monkeypatch):
         s.close()
     assert np.array_equal(outs[0][0], outs[1][0])
     assert outs[0][1] < outs[1][1]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_no_write_outside_the_f_buffers(dtype):
+    """Guard bands around caller-owned buffers (compute-sanitizer is closed on this pool): every
+    kernel family on ragged sizes (tiles, chunks and segments that do not divide evenly) must leave
+    the sentinels on both sides of both buffers untouched."""
+    import torch
+    from paper_1907_08316_b200.sldg import Sldg
+    G = 4096
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    for dx, dv, cells, o in ((2, 2, (11, 7, 9, 5), 3), (3, 3, (5, 3, 4, 3, 5, 3), 2), (1, 1, (37, 29), 4),
+                             (2, 2, (10, 6, 7, 5), 2)):
+        cfg = W.Config("g", dx, dv, cells, o, (0.0,) * (dx + dv), tuple(float(c) for c in cells), dt=0.1)
+        n = cfg.ndof
+        big = [torch.full((n + 2 * G,), -777.0, dtype=tdt, device="cuda") for _ in range(2)]
+        bufs = [b[G:G + n] for b in big]
+        s = Sldg(cfg.dx, cfg.dv, cfg.cells, cfg.order, cfg.lo, cfg.hi, dtype=dtype, buffers=bufs)
+        s.fill_uniform(W.SEED, 0)
+        rng = np.random.default_rng(1)
+        D = dx + dv
+        sig = [torch.from_numpy(rng.uniform(-3.5, 3.5, cfg.N[dx + k] if k < dx else cfg.X)).cuda() for k in range(D)]
+        for k in range(D):
+            s.translate(k, sig[k])
+        s.translate_pair(0, sig[0], 1, sig[1]) if dx >= 2 else None
+        s.translate_pair(dx, sig[dx], dx + 1, sig[dx + 1]) if dv >= 2 else None
+        if dx == 3:
+            s.translate_triple(0, sig[0], 1, sig[1], 2, sig[2])
+            s.translate_triple(3, sig[3], 4, sig[4], 5, sig[5])
+        s.step(0.1)
+        s.diagnostics()
+        s.moments()
+        torch.cuda.synchronize()
+        for b in big:
+            assert bool((b[:G] == -777.0).all()) and bool((b[G + n:] == -777.0).all()), (cells, o)
+        assert bool(torch.isfinite(s.current()).all())
+        s.close()
