@@ -384,7 +384,7 @@ namespace {
 template <typename T, int O, int VEC, bool QV>
 void launch_strided(sldg_ctx *c, const T *in, T *out, long inner, int n, long outer, long count,
                     long qdiv, long qmod) {
-    constexpr int UB = (O <= 3) ? 4 : 2;
+    constexpr int UB = (O <= 4) ? 4 : 2;
     long lines_v = outer * (inner / VEC);
     // split lines into segments only when there are too few of them to fill the machine
     long target = (long)c->sm_count * 2048;
@@ -429,7 +429,11 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
         bool done = false;
         if (c->use_tma && line_bytes % 16 == 0 && line_bytes <= 96 * 1024) {
             // staged variant: R whole lines per block through shared memory (bulk copies)
-            long R = (32 * 1024) / (long)line_bytes;
+            // chunk per block: 32 KB (o <= 3) / 16 KB with 128-thread blocks (o >= 4: the per-cell
+            // arithmetic needs ~95+ registers, and only more, smaller blocks keep enough copies in flight)
+            const long chunk_bytes = (O <= 3) ? 32 * 1024 : 16 * 1024;
+            const int max_block = (O <= 3) ? 256 : 128;
+            long R = chunk_bytes / (long)line_bytes;
             if (R < 1) R = 1;
             if (R > qdiv) R = qdiv;
             int chunks = (int)cdiv(qdiv, R);
@@ -441,7 +445,7 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
                 attr_set = 200 * 1024;
             }
             long ncell = R * n;
-            int block = ncell >= 256 ? 256 : (int)(cdiv(ncell, 32) * 32);
+            int block = ncell >= max_block ? max_block : (int)(cdiv(ncell, 32) * 32);
             if (block < 64) block = 64;
             sweep_x1_bulk_kernel<T, O><<<(unsigned)(ngroups * chunks), block, smem, c->stream>>>(
                 in, out, n, qdiv, (int)R, chunks, c->d_m, (const T *)c->d_ab, count, c->N[c->dx]);
