@@ -18,6 +18,7 @@
 // contiguous x_1 line (k1 = 0).
 #pragma once
 #include "sweep.cuh"
+#include "tma.cuh"
 
 namespace sldg {
 
@@ -177,7 +178,7 @@ namespace sldg {
 // and one write of f for three sweeps.  Instantiated for O <= 2 (4 O^3 raw values per cell).
 // ------------------------------------------------------------------------------------------
 template <typename T, int O, bool VEC1>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 3)
 sweep_triple_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, int n1, long mid12, int n2,
                     long mid23, int n3, long outer3, int chunk,
                     const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
@@ -269,18 +270,46 @@ sweep_triple_kernel(const T *__restrict__ in, T *__restrict__ out, long inner1, 
         }
     };
 
+    // x-triple (VEC1: k1 = x_1 contiguous, k2 = x_2 adjacent): the raw rows of one k3-cell that
+    // this thread's k2-cell pair needs are two contiguous spans of O x_1-lines per k3-row; the
+    // owner of c1 == 0 asks the copy engine to pull them into L2 two k3-cells ahead, so the
+    // demand loads (one cell ahead, in registers) find them in L2 instead of HBM.
+    auto prefetch_l2 = [&](int cell3) {
+        if constexpr (VEC1) {
+            if (c1 == 0 && mid12 == 1) {
+                const uint32_t span = (uint32_t)((size_t)O * s2 * sizeof(T));
+#pragma unroll
+                for (int l3 = 0; l3 < O; ++l3) {
+                    const T *row = in + base + ((long)cell3 * O + l3) * s3;
+                    bulk_prefetch_l2(row + (long)sa2 * O * s2, span);
+                    bulk_prefetch_l2(row + (long)sb2 * O * s2, span);
+                }
+            }
+        }   // (per-lane bulk prefetches in the strided v-triple were tried: 16.6 -> 23.0 ms, removed)
+    };
+
     int is3 = m3;                                            // source k3-cell of output cell 0
     T raw[O][2][O][2][O], w0[O][O][O], w1[O][O][O];
     load_raw(is3, raw);
     k12_rule(raw, w0);
     if (++is3 == n3) is3 = 0;
     load_raw(is3, raw);
+    {
+        int p3 = is3 + 1;
+        if (p3 == n3) p3 = 0;
+        prefetch_l2(p3);
+    }
     T *dst = out + lin0;
     for (int i3 = 0; i3 < n3; ++i3) {
         k12_rule(raw, w1);
         if (i3 + 1 < n3) {                                   // next cell's loads fly during the arithmetic below
             if (++is3 == n3) is3 = 0;
             load_raw(is3, raw);
+            if (i3 + 2 < n3) {
+                int p3 = is3 + 1;
+                if (p3 == n3) p3 = 0;
+                prefetch_l2(p3);
+            }
         }
 #pragma unroll
         for (int j3 = 0; j3 < O; ++j3)
