@@ -59,16 +59,6 @@ __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.
 // generic-proxy writes to shared memory -> visible to the async proxy (before a bulk store)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// tiled 3-D tensor load: box at coordinates (c0 fastest, c1, c2) -> shared
-__device__ __forceinline__ void tma_load_3d(void *smem_dst, const CUtensorMap *tmap, int c0, int c1, int c2,
-                                            uint64_t *bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, "
-        "%4}], [%5];" ::"r"(smem_u32(smem_dst)),
-        "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
-        : "memory");
-}
-
 // ---- L2 cache policies (createpolicy) and hinted accesses ------------------------------------
 __device__ __forceinline__ uint64_t policy_evict_last() {
     uint64_t p;
@@ -95,6 +85,7 @@ __device__ __forceinline__ int ld_hint(const int *p, uint64_t pol) {
     asm volatile("ld.global.nc.L2::cache_hint.s32 %0, [%1], %2;" : "=r"(v) : "l"(p), "l"(pol));
     return v;
 }
+// tiled 3-D tensor load with an L2 cache policy: box at coordinates (c0 fastest, c1, c2) -> shared
 __device__ __forceinline__ void tma_load_3d_hint(void *smem_dst, const CUtensorMap *tmap, int c0, int c1, int c2,
                                                  uint64_t *bar, uint64_t pol) {
     asm volatile(
