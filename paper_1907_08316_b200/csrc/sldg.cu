@@ -72,6 +72,22 @@ struct sldg_ctx {
     double *d_t[4] = {nullptr, nullptr, nullptr, nullptr};   // complex scratch (re, im) x 2
     double *d_gh[2] = {nullptr, nullptr};                    // g_hat (re, im) [KK]
 
+    // CUDA graphs for launch-bound (small) problems: the kernels of one Strang step captured once per
+    // (dt, buffer parity) on an internal stream and replayed on the caller's stream (SLDG_NO_GRAPH=1: off)
+    struct StepGraph {
+        cudaGraphExec_t exec = nullptr;
+        double dt = 0.0;
+        int cur_in = -1, cur_out = 0;
+        unsigned long long launches = 0;
+        unsigned long long xt_epoch = 0;   // the cached x-tables the captured kernels read
+    };
+    StepGraph graphs[2];
+    unsigned long long xt_epoch = 0;       // bumped whenever a cached x-table is rewritten
+    cudaStream_t capture_stream = nullptr;
+    bool use_graph = true;
+    double last_eager_dt[2] = {0.0, 0.0};   // dt of the last eager step that started from parity 0 / 1
+    bool eager_seen[2] = {false, false};
+    unsigned long long eager_epoch[2] = {0, 0};   // xt_epoch right after that eager step
     bool use_fuse = true;              // SLDG_NO_FUSE=1: sldg_step issues one sweep per pass
     bool use_tma = true;               // SLDG_NO_TMA=1 in the environment selects the plain kernels
     bool have_rho = false, have_E = false;
@@ -193,6 +209,8 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         c->use_tma = !(e && e[0] == '1');
         e = getenv("SLDG_NO_FUSE");
         c->use_fuse = !(e && e[0] == '1');
+        e = getenv("SLDG_NO_GRAPH");
+        c->use_graph = !(e && e[0] == '1') && c->ndof <= (1L << 24);
     }
     int dev = 0;
     cudaGetDevice(&dev);
@@ -337,6 +355,8 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
 extern "C" int sldg_destroy(sldg_ctx *ctx) {
     if (!ctx) return SLDG_ERR_ARG;
     cudaStreamSynchronize(ctx->stream);
+    for (auto &g : ctx->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
+    if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
     free_tables(ctx);
     delete ctx;
     return SLDG_OK;
@@ -702,6 +722,7 @@ int physics_tab(sldg_ctx *c, int slot, int dim, double dt) {
             c->d_coords[va], count, dt, c->h[dim], t.sigma);
         t.tau = dt;
         t.valid = true;                 // the assembly is enqueued by the sweep that follows
+        c->xt_epoch++;
     } else {
         int a = dim - c->dx;
         if (a >= c->dx) return fail(c, SLDG_ERR_ARG, "sldg_advect: v_%d has no field component (dx = %d)", a + 1, c->dx);
@@ -943,8 +964,8 @@ int advect_group(sldg_ctx *c, int base, int cnt, double tau) {
 }
 }  // namespace
 
-extern "C" int sldg_step(sldg_ctx *c, double dt) {
-    if (!c) return SLDG_ERR_ARG;
+namespace {
+int step_body(sldg_ctx *c, double dt) {
     int rc;
     if ((rc = advect_group(c, 0, c->dx, 0.5 * dt))) return rc;
     if ((rc = run_rho(c, nullptr, false))) return rc;
@@ -952,6 +973,58 @@ extern "C" int sldg_step(sldg_ctx *c, double dt) {
     if ((rc = advect_group(c, c->dx, c->dx, dt))) return rc;
     if ((rc = advect_group(c, 0, c->dx, 0.5 * dt))) return rc;
     return SLDG_OK;
+}
+
+// Capture one step (starting from the current buffer parity) into an executable graph.  Nothing runs
+// during the capture; the context's bookkeeping advances exactly as in an eager step.
+int capture_step(sldg_ctx *c, double dt, sldg_ctx::StepGraph &g) {
+    if (!c->capture_stream)
+        CUDA_TRY(c, cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking));
+    if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+    cudaStream_t user = c->stream;
+    const int cur_in = c->cur;
+    const unsigned long long l0 = c->launches;
+    CUDA_TRY(c, cudaStreamBeginCapture(c->capture_stream, cudaStreamCaptureModeThreadLocal));
+    c->stream = c->capture_stream;
+    int rc = step_body(c, dt);
+    c->stream = user;
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->capture_stream, &graph);
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(c, SLDG_ERR_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+    e = cudaGraphInstantiate(&g.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { g.exec = nullptr; return fail(c, SLDG_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e)); }
+    g.dt = dt; g.cur_in = cur_in; g.cur_out = c->cur; g.launches = c->launches - l0;
+    g.xt_epoch = c->xt_epoch;
+    return SLDG_OK;
+}
+}  // namespace
+
+extern "C" int sldg_step(sldg_ctx *c, double dt) {
+    if (!c) return SLDG_ERR_ARG;
+    if (!c->use_graph) return step_body(c, dt);
+    const int p = c->cur;
+    sldg_ctx::StepGraph &g = c->graphs[p];
+    if (g.exec && g.dt == dt && g.cur_in == p && g.xt_epoch == c->xt_epoch) {   // replay
+        CUDA_TRY(c, cudaGraphLaunch(g.exec, c->stream));
+        c->cur = g.cur_out; c->launches += g.launches;
+        c->have_rho = false; c->have_E = true;
+        return SLDG_OK;
+    }
+    if (c->eager_seen[p] && c->last_eager_dt[p] == dt && c->eager_epoch[p] == c->xt_epoch) {
+        // second step with this (dt, parity) and untouched x-tables: capture (no table kernels inside)
+        int rc = capture_step(c, dt, g);
+        if (rc) return rc;
+        CUDA_TRY(c, cudaGraphLaunch(g.exec, c->stream));
+        return SLDG_OK;
+    }
+    // first step with this (dt, parity): eager (it also fills the cached x-tables and kernel attributes)
+    c->eager_seen[p] = true;
+    c->last_eager_dt[p] = dt;
+    int rc = step_body(c, dt);
+    c->eager_epoch[p] = c->xt_epoch;
+    return rc;
 }
 
 namespace {

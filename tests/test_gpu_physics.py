@@ -226,3 +226,27 @@ def test_paper_twostream_fp32_vs_fp64_reduced():
     assert out["max_rel_ee_diff_vs_trace_max"] < 2e-4
     assert out["mass_drift64"] < 1e-12 and out["mass_drift32"] < 1e-5
     assert out["energy_drift64"] < 1e-2
+
+
+def test_graph_replay_equals_eager_and_survives_interleaved_calls(monkeypatch):
+    """Small problems replay a captured CUDA graph of the step; results must be bit-identical to
+    eager stepping, also when other sweeps (other tau: the cached x-tables change) come in between."""
+    cfg = W.CONFIG2.scaled((48, 40))
+    outs = []
+    for flag in ("0", "1"):
+        monkeypatch.setenv("SLDG_NO_GRAPH", flag)
+        s = make_solver(cfg, "f64")
+        s.set_initial(W.initial_state(cfg, [s.node_coords(0), s.node_coords(1)]))
+        l0 = s.launch_count()
+        for n in range(12):
+            s.step(cfg.dt)
+            if n == 5:
+                s.advect(0, 0.0123)             # rewrites the cached x-table (different tau)
+                s.diagnostics()
+            if n == 8:
+                s.step(0.5 * cfg.dt)            # another dt in between
+        outs.append((s.get_f(), s.diagnostics(), s.launch_count() - l0))
+        s.close()
+    assert np.array_equal(outs[0][0], outs[1][0])
+    assert outs[0][1] == outs[1][1]
+    assert outs[0][2] == outs[1][2]                 # the launch count is kept in step with replays
