@@ -14,7 +14,7 @@ def _line_matrices(oracle, o, sigma, dtype=np.float64):
 # ---------------------------------------------------------------- P4: integer shifts are exact
 
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
-@pytest.mark.parametrize("o", [1, 2, 3, 4])
+@pytest.mark.parametrize("o", [1, 2, 3, 4, 5, 6])
 def test_P4_integer_shift_is_a_bit_exact_roll(oracle, o, dtype):
     rng = np.random.default_rng(1)
     n = 7
@@ -77,7 +77,7 @@ def _brute_force_line(o, n, sigma, u):
     return out
 
 
-@pytest.mark.parametrize("o,sigma", [(2, 0.3), (2, -1.6), (3, 0.45), (3, -0.2), (4, 2.25)])
+@pytest.mark.parametrize("o,sigma", [(2, 0.3), (2, -1.6), (3, 0.45), (3, -0.2), (4, 2.25), (5, 0.37), (6, -0.7)])
 def test_P11_brute_force_projection(oracle, o, sigma):
     rng = np.random.default_rng(o * 100 + 7)
     n = 4
@@ -90,7 +90,7 @@ def test_P11_brute_force_projection(oracle, o, sigma):
 
 # ---------------------------------------------------------------- P7: polynomial reproduction
 
-@pytest.mark.parametrize("o", [2, 3, 4])
+@pytest.mark.parametrize("o", [2, 3, 4, 5, 6])
 def test_P7_polynomials_below_order_are_reproduced(oracle, o):
     n = 16
     xr, _ = np_gl01(o)
@@ -107,7 +107,7 @@ def test_P7_polynomials_below_order_are_reproduced(oracle, o):
     u = (x / n) ** o
     un = oracle.translate_line(o, A, B, m, u)
     err = np.max(np.abs(un - ((x - sigma) / n) ** o)[interior])
-    assert 1e-9 < err < 1e-2
+    assert 1e-12 < err < 1e-2          # (1.4e-11 at o = 6 on 16 cells; round-off is 5e-15)
 
 
 def test_sign_of_the_shift(oracle):
@@ -125,7 +125,7 @@ def test_sign_of_the_shift(oracle):
 # ---------------------------------------------------------------- P5 / P8: mass and L2
 
 @pytest.mark.parametrize("dtype,tol", [(np.float64, 2e-15), (np.float32, 2e-7)])
-@pytest.mark.parametrize("o", [2, 3, 4])
+@pytest.mark.parametrize("o", [2, 3, 4, 5, 6])
 def test_P5_P8_mass_conserved_l2_contracts(oracle, o, dtype, tol):
     rng = np.random.default_rng(5)
     n = 24
