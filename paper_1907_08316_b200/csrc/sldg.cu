@@ -647,6 +647,27 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
             qm[i] = c->N[c->dx + ks[i]];
         } else { qd[i] = 1; qm[i] = c->X; }
     }
+    // x_1 x_2 x_3 with a small x-grid: copy-engine staged plane kernel, one block per velocity node
+    {
+        const size_t slab_bytes = (size_t)O * n2 * O * n1 * O * sizeof(T);
+        const size_t slot = (slab_bytes + 127) & ~(size_t)127;
+        if (c->use_tma && k1 == 0 && k2 == 1 && k3 == 2 && c->dx == 3 && slab_bytes % 16 == 0 &&
+            3 * slot <= 200 * 1024 && (long)n1 * n2 <= 512 && outer3 < (1L << 31)) {
+            static bool attr_set = false;
+            if (!attr_set) {
+                cudaFuncSetAttribute(sweep_xtriple_plane_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+                attr_set = true;
+            }
+            int block = (int)(cdiv((long)n1 * n2, 32) * 32);
+            sweep_xtriple_plane_kernel<T, O><<<(unsigned)outer3, block, 3 * slot, c->stream>>>(
+                in, out, n1, n2, n3, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2,
+                qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+            LAUNCH_CHECK(c);
+            c->cur ^= 1;
+            c->have_rho = false;
+            return SLDG_OK;
+        }
+    }
     int chunk = 32;
     while (inner1 % chunk) chunk /= 2;
     long threads = inner1 * n1 * mid12 * n2 * mid23 * outer3;
