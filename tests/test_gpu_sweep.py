@@ -252,8 +252,12 @@ def test_ab_tables_are_rounded_once(oracle, o):
     got = s.get_f()
     s.close()
     ref = oracle.translate(f0.copy(), cfg.N, o, 0, -theta, [1])
-    assert np.max(np.abs(got - ref)) <= 2.3e-16 * max(1.0, np.max(np.abs(ref)))
-    assert np.mean(got != ref) < 0.02                 # and almost always the very same double
+    nz = ref != 0.0
+    assert np.array_equal(got == 0.0, ref == 0.0)
+    # at most one ulp of the entry; entries that are tiny by cancellation (A near theta = 1, B near 0)
+    # carry the oracle's long-double ABSOLUTE error of a few 1e-19 of the O(1) terms they are summed from
+    assert np.all(np.abs(got - ref)[nz] <= np.spacing(np.abs(ref[nz])) + 2e-18)
+    assert np.mean(got[nz] != ref[nz]) < 0.05                                   # and almost always the same double
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
