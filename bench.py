@@ -439,6 +439,12 @@ def run_ours(args):
                 steps_tab[c2.name] = strang_step_table(torch, Sldg, c2, "f64", nst)
             except Exception as exc:
                 steps_tab[c2.name] = {"error": str(exc)}
+        if args.workload == "config4":          # the paper's section-7 set-ups (1+3 D, 2+3 D at o = 4), context only
+            for c2 in (W.MIXED13, W.MIXED23):
+                try:
+                    steps_tab[c2.name] = strang_step_table(torch, Sldg, c2, "f64", c2.steps)
+                except Exception as exc:
+                    steps_tab[c2.name] = {"error": str(exc)}
         line["strang_steps_fused"] = steps_tab
 
     # ---- the oracle on the host cores, bounded sample (rank 0, N = 1 only)

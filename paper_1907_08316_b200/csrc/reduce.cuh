@@ -70,21 +70,30 @@ vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
     }
 }
 
-// rho[x] = -sum_split part_rho[split][x] (fixed order);  s2[x] = +sum_split part_s2[split][x]
-__global__ void vsum_final_kernel(const double *__restrict__ part_rho,
-                                  const double *__restrict__ part_s2, long X, int splits,
-                                  double *__restrict__ rho, double *__restrict__ rho_copy,
-                                  double *__restrict__ s2) {
-    long x = (long)blockIdx.x * blockDim.x + threadIdx.x;
+__device__ __forceinline__ double warp_sum(double v);
+
+// rho[x] = -sum_split part_rho[split][x];  s2[x] = +sum_split part_s2[split][x].
+// One WARP per x: lane l adds splits l, l+32, ... in ascending order, then a fixed shuffle tree
+// (deterministic; with one split it is exactly the single partial).  A thread per x walking
+// thousands of splits serially made this pass slower than the partial pass for small X (1+3 D).
+__global__ void __launch_bounds__(256)
+vsum_final_kernel(const double *__restrict__ part_rho, const double *__restrict__ part_s2, long X, int splits,
+                  double *__restrict__ rho, double *__restrict__ rho_copy, double *__restrict__ s2) {
+    const long x = ((long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
     if (x >= X) return;
     double a = 0.0, b = 0.0;
-    for (int s = 0; s < splits; ++s) {
+    for (int s = lane; s < splits; s += 32) {
         a += part_rho[(long)s * X + x];
         if (part_s2) b += part_s2[(long)s * X + x];
     }
-    rho[x] = -a;
-    if (rho_copy) rho_copy[x] = -a;
-    if (s2) s2[x] = b;
+    a = warp_sum(a);
+    b = warp_sum(b);
+    if (lane == 0) {
+        rho[x] = -a;
+        if (rho_copy) rho_copy[x] = -a;
+        if (s2) s2[x] = b;
+    }
 }
 
 __device__ __forceinline__ double warp_sum(double v) {

@@ -309,7 +309,7 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         long smax = c->V / 16 > 0 ? c->V / 16 : 1;
         if (s > smax) s = smax;
         if (s < 1) s = 1;
-        if (s > 1024) s = 1024;
+        if (s > 8192) s = 8192;
         c->max_splits = (int)s;
         CREATE_TRY(dalloc(&c->d_part, (size_t)4 * c->max_splits * c->X));
     }
@@ -453,10 +453,17 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
             // arithmetic needs ~95+ registers, and only more, smaller blocks keep enough copies in flight)
             const long chunk_bytes = (O <= 3) ? 32 * 1024 : 16 * 1024;
             const int max_block = (O <= 3) ? 256 : 128;
+            // shift groups: d_x >= 2: qdiv contiguous lines per (v_1 node, rest); d_x = 1: the lines of one
+            // v_1 node are N_v1 lines apart (group = v_1 node, outer / N_v1 strided lines)
+            const bool strided_group = (qdiv == 1 && outer > c->N[c->dx]);
+            const long lpg = strided_group ? outer / c->N[c->dx] : qdiv;          // lines per group
+            const long groups = strided_group ? c->N[c->dx] : ngroups;
+            const long group_stride = strided_group ? (long)n * O : qdiv * (long)n * O;
+            const long line_stride = strided_group ? c->N[c->dx] * (long)n * O : (long)n * O;
             long R = chunk_bytes / (long)line_bytes;
             if (R < 1) R = 1;
-            if (R > qdiv) R = qdiv;
-            int chunks = (int)cdiv(qdiv, R);
+            if (R > lpg) R = lpg;
+            int chunks = (int)cdiv(lpg, R);
             size_t half = ((size_t)R * line_bytes + 127) & ~(size_t)127;
             size_t smem = 2 * half;
             static size_t attr_set = 0;
@@ -467,8 +474,9 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
             long ncell = R * n;
             int block = ncell >= max_block ? max_block : (int)(cdiv(ncell, 32) * 32);
             if (block < 64) block = 64;
-            sweep_x1_bulk_kernel<T, O><<<(unsigned)(ngroups * chunks), block, smem, c->stream>>>(
-                in, out, n, qdiv, (int)R, chunks, c->d_m, (const T *)c->d_ab, count, c->N[c->dx]);
+            sweep_x1_bulk_kernel<T, O><<<(unsigned)(groups * chunks), block, smem, c->stream>>>(
+                in, out, n, lpg, (int)R, chunks, c->d_m, (const T *)c->d_ab, count, c->N[c->dx], group_stride,
+                line_stride);
             done = true;
         }
         if (!done) {
@@ -839,7 +847,7 @@ int run_vsum(sldg_ctx *c, double *rho_copy) {
     else launch_vsum<T, 1, S2, 8>(c, splits, vps, 128);
     LAUNCH_CHECK(c);
     int block = 256;
-    vsum_final_kernel<<<(unsigned)cdiv(c->X, block), block, 0, c->stream>>>(
+    vsum_final_kernel<<<(unsigned)cdiv(c->X * 32, block), block, 0, c->stream>>>(
         c->d_part, S2 ? c->d_part + (size_t)c->max_splits * c->X : nullptr, c->X, splits, c->d_rho,
         rho_copy, S2 ? c->d_s2 : nullptr);
     LAUNCH_CHECK(c);

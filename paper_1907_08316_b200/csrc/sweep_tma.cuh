@@ -107,7 +107,7 @@ template <typename T, int O>
 __global__ void __launch_bounds__(256)
 sweep_x1_bulk_kernel(const T *__restrict__ in, T *__restrict__ out, int n, long lines_per_group, int R,
                      int chunks_per_group, const int *__restrict__ mtab, const T *__restrict__ ab,
-                     long count, long qmod) {
+                     long count, long qmod, long group_stride, long line_stride) {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar;
     __shared__ T s_ab[2 * O * O];
@@ -122,13 +122,19 @@ sweep_x1_bulk_kernel(const T *__restrict__ in, T *__restrict__ out, int n, long 
     const size_t half = ((size_t)R * n * O * sizeof(T) + 127) & ~(size_t)127;
     T *s_in = reinterpret_cast<T *>(smem_raw);
     T *s_out = reinterpret_cast<T *>(smem_raw + half);
-    const long base = (g * lines_per_group + line0) * (long)n * O;
+    // lines of a shift group: contiguous (d_x >= 2: line_stride == n*O, one copy for the whole chunk) or
+    // strided (d_x = 1: the lines that share a v_1 node are N_v1 lines apart; one copy per line)
+    const long base = g * group_stride + line0 * line_stride;
+    const bool contiguous = line_stride == (long)n * O;
+    const uint32_t line_bytes = (uint32_t)((size_t)n * O * sizeof(T));
 
-    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_expect_tx(&bar, bytes); }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        mbar_expect_tx(&bar, bytes);
-        bulk_g2s(s_in, in + base, bytes, &bar);
+    if (contiguous) {
+        if (threadIdx.x == 0) bulk_g2s(s_in, in + base, bytes, &bar);
+    } else {
+        for (int r = threadIdx.x; r < nl; r += blockDim.x)
+            bulk_g2s(s_in + (size_t)r * n * O, in + base + r * line_stride, line_bytes, &bar);
     }
     const long q = g % qmod;
     for (int e = threadIdx.x; e < 2 * O * O; e += blockDim.x) s_ab[e] = ab[(long)e * count + q];
@@ -168,10 +174,18 @@ sweep_x1_bulk_kernel(const T *__restrict__ in, T *__restrict__ out, int n, long 
     }
     fence_proxy_async();
     __syncthreads();
-    if (threadIdx.x == 0) {
-        bulk_s2g(out + base, s_out, bytes);
-        bulk_commit();
-        bulk_wait_read0();
+    if (contiguous) {
+        if (threadIdx.x == 0) {
+            bulk_s2g(out + base, s_out, bytes);
+            bulk_commit();
+            bulk_wait_read0();
+        }
+    } else {
+        for (int r = threadIdx.x; r < nl; r += blockDim.x) {
+            bulk_s2g(out + base + r * line_stride, s_out + (size_t)r * n * O, line_bytes);
+            bulk_commit();
+            bulk_wait_read0();
+        }
     }
 }
 

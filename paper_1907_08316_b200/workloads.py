@@ -86,6 +86,13 @@ PAPER_TWOSTREAM = Config("paper-twostream-2+2", 2, 2, (60, 60, 60, 60), 4, (0.0,
                          (10 * _PI, 10 * _PI, 6.0, 6.0), dt=0.1, steps=1000, kind="twostream2",
                          eps=1e-3, k=0.2, extra={"v0": 2.4})
 
+# S:8(f) NEXT-3 -- the mixed-dimension set-ups of the paper's section 7 (1+3 D and 2+3 D at o = 4; the
+# paper's grid sizes are lost with its figures: these are this build's choices, ~1e9 and ~3.6e9 DOF).
+MIXED13 = Config("mixed-landau-1+3", 1, 3, (32, 48, 48, 48), 4, (0.0, -6.0, -6.0, -6.0),
+                 (4 * _PI, 6.0, 6.0, 6.0), dt=0.1, steps=5, kind="landau", eps=0.01, k=0.5)
+MIXED23 = Config("mixed-landau-2+3", 2, 3, (16, 16, 24, 24, 24), 4, (0.0, 0.0, -6.0, -6.0, -6.0),
+                 (4 * _PI, 4 * _PI, 6.0, 6.0, 6.0), dt=0.1, steps=3, kind="landau", eps=0.01, k=0.5)
+
 CONFIGS = {c.name.split("-")[0]: c for c in (CONFIG1, CONFIG2, CONFIG3, CONFIG4, CONFIG5)}
 
 
