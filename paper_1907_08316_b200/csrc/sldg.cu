@@ -597,6 +597,29 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
     long threads = lines * nseg;
     int chunk = 32;
     while (inner1 % chunk) chunk /= 2;
+    // x_1 x_2: copy-engine staged plane kernel, one block per (x_1, x_2) plane
+    {
+        const size_t slab_bytes = (size_t)O * n1 * O * sizeof(T);
+        const size_t slot = (slab_bytes + 127) & ~(size_t)127;
+        const long planes = midN * outer2;           // midN == 1 for (0, 1)
+        const char *e = getenv("SLDG_NO_PLANE_PAIR");
+        if (c->use_tma && !(e && e[0] == '1') && k1 == 0 && k2 == 1 && slab_bytes % 16 == 0 && 3 * slot <= 96 * 1024 &&
+            n1 <= 256 && n2 >= 3 && planes < (1L << 31)) {
+            static bool attr_set = false;
+            if (!attr_set) {
+                cudaFuncSetAttribute(sweep_xpair_plane_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+                attr_set = true;
+            }
+            int blk = (int)(cdiv(n1, 32) * 32);
+            sweep_xpair_plane_kernel<T, O><<<(unsigned)planes, blk, 3 * slot, c->stream>>>(
+                in, out, n1, n2, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2, (const T *)c->d_ab2, count2,
+                qd2, qm2);
+            LAUNCH_CHECK(c);
+            c->cur ^= 1;
+            c->have_rho = false;
+            return SLDG_OK;
+        }
+    }
     // (the vectorised-cell variant VEC1 helps the triple kernel but measured slower for the pair
     //  kernel at config 3: 0.906 vs 0.704 ms, so the pair always uses scalar accesses)
     sweep_pair_kernel<T, O, false><<<(unsigned)cdiv(threads, 128), 128, 0, c->stream>>>(

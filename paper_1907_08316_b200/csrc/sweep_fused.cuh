@@ -498,3 +498,122 @@ sweep_xtriple_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1
 }
 
 }  // namespace sldg
+
+namespace sldg {
+
+// ------------------------------------------------------------------------------------------
+// x_1 x_2 pair, STAGED BY THE COPY ENGINE (the pair analogue of sweep_xtriple_plane_kernel).
+// One block per (x_1, x_2) plane, i.e. per value of all higher indices; its shifts and A,B are
+// uniform (they depend on v only).  A k2-cell of the plane is ONE contiguous slab of O * N1
+// values, streamed through a 3-deep shared-memory ring by cp.async.bulk; thread c1 reads its two
+// source cells from the slab, keeps its O x O window along x_2 and emits O x O outputs per cell.
+// No raw-value registers and no register prefetch: at o = 3, 4 the register pair kernel is
+// occupancy-starved (168 / 255 registers), this one is not.
+// ------------------------------------------------------------------------------------------
+template <typename T, int O>
+__global__ void __launch_bounds__(256)
+sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2,
+                         const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
+                         const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t full[3];
+    const long N1 = (long)n1 * O;
+    const long slab = O * N1;                                // elements per k2-cell of one plane
+    const size_t slab_bytes = (size_t)slab * sizeof(T);
+    const size_t slot_stride = (slab_bytes + 127) & ~(size_t)127;
+    const long base = (long)blockIdx.x * n2 * slab;          // planes are contiguous
+    const int tid = threadIdx.x;
+    const int c1 = tid;
+    const bool active = c1 < n1;
+
+    const long q1 = (base / qdiv1) % qmod1, q2 = (base / qdiv2) % qmod2;
+    T A1[O * O], B1[O * O], A2[O * O], B2[O * O];
+#pragma unroll
+    for (int e = 0; e < O * O; ++e) {
+        A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1];
+        A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
+    }
+    const int m1 = mtab1[q1], m2 = mtab2[q2];
+    int sa1 = (active ? c1 : 0) + m1; if (sa1 >= n1) sa1 -= n1;
+    int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < 3; ++s) mbar_init(&full[s], 1);
+    }
+    __syncthreads();
+    auto issue = [&](int j) {                                // slab j <-> source k2-cell (m2 + j) mod n2
+        int cell = m2 + j;
+        if (cell >= n2) cell -= n2;
+        const int slot = j % 3;
+        mbar_expect_tx(&full[slot], (uint32_t)slab_bytes);
+        bulk_g2s(smem_raw + slot * slot_stride, in + base + (long)cell * slab, (uint32_t)slab_bytes, &full[slot]);
+    };
+    if (tid == 0)
+        for (int j = 0; j < 3 && j < n2; ++j) issue(j);
+
+    auto k1_from_slab = [&](int slot, T (&w)[O][O]) {       // w[l2][j1]
+        const T *sl = reinterpret_cast<const T *>(smem_raw + slot * slot_stride);
+#pragma unroll
+        for (int l2 = 0; l2 < O; ++l2) {
+            T r0[O], r1[O];
+            load_cell<T, O>(sl + l2 * N1 + (long)sa1 * O, r0);
+            load_cell<T, O>(sl + l2 * N1 + (long)sb1 * O, r1);
+#pragma unroll
+            for (int j1 = 0; j1 < O; ++j1) w[l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+        }
+    };
+    auto emit = [&](int i2, const T (&w0)[O][O], const T (&w1)[O][O]) {
+        T *dst = out + base + (long)i2 * slab + (long)c1 * O;
+#pragma unroll
+        for (int j2 = 0; j2 < O; ++j2) {
+            T res[O];
+#pragma unroll
+            for (int j1 = 0; j1 < O; ++j1) {
+                T a0[O], a1[O];
+#pragma unroll
+                for (int l = 0; l < O; ++l) { a0[l] = w0[l][j1]; a1[l] = w1[l][j1]; }
+                res[j1] = chain<T, O>(A2, B2, j2, a0, a1);
+            }
+            T *p = dst + (long)j2 * N1;
+            if constexpr (O % 2 == 0) {
+                using V2 = Vec<T, 2>;
+#pragma unroll
+                for (int j1 = 0; j1 < O; j1 += 2) {
+                    V2 vv; vv.v[0] = res[j1]; vv.v[1] = res[j1 + 1];
+                    *reinterpret_cast<V2 *>(p + j1) = vv;
+                }
+            } else {
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) p[j1] = res[j1];
+            }
+        }
+    };
+
+    T wfirst[O][O], w0[O][O], w1[O][O];
+    for (int j = 0; j < n2; ++j) {
+        const int slot = j % 3;
+        mbar_wait(&full[slot], (uint32_t)((j / 3) & 1));
+        if (active) {
+            if (j == 0) {
+                k1_from_slab(slot, wfirst);
+#pragma unroll
+                for (int a = 0; a < O; ++a)
+#pragma unroll
+                    for (int b = 0; b < O; ++b) w0[a][b] = wfirst[a][b];
+            } else {
+                k1_from_slab(slot, w1);
+                emit(j - 1, w0, w1);
+#pragma unroll
+                for (int a = 0; a < O; ++a)
+#pragma unroll
+                    for (int b = 0; b < O; ++b) w0[a][b] = w1[a][b];
+            }
+        }
+        __syncthreads();                                     // everyone is done with this slot
+        if (tid == 0 && j + 3 < n2) issue(j + 3);
+    }
+    if (active) emit(n2 - 1, w0, wfirst);                    // closes the periodic line
+}
+
+}  // namespace sldg
