@@ -250,3 +250,27 @@ def test_graph_replay_equals_eager_and_survives_interleaved_calls(monkeypatch):
     assert np.array_equal(outs[0][0], outs[1][0])
     assert outs[0][1] == outs[1][1]
     assert outs[0][2] == outs[1][2]                 # the launch count is kept in step with replays
+
+
+def test_config2_fp32_vs_fp64_on_the_gpu():
+    """BASELINE.json configs[1]: 'compare fp32 vs fp64 electric-energy trace' (reported; the paper's
+    own fp32-vs-fp64 bound for its 2+2 D two-stream run, 2e-4, is the context -- PAPER.md line 235)."""
+    cfg = W.CONFIG2
+    runs = {}
+    for dtype in ("f64", "f32"):
+        s = make_solver(cfg, dtype)
+        s.set_initial(W.initial_state(cfg, [s.node_coords(0), s.node_coords(1)], NPDT[dtype]))
+        tr = [s.diagnostics()]
+        for _ in range(cfg.steps):
+            s.step(cfg.dt)
+            tr.append(s.diagnostics())
+        runs[dtype] = (s.get_f().astype(np.float64), np.array(tr))
+        s.close()
+    f64, t64 = runs["f64"]
+    f32, t32 = runs["f32"]
+    df = np.max(np.abs(f32 - f64)) / np.max(np.abs(f64))
+    dee = np.max(np.abs(t32[:, 2] - t64[:, 2])) / np.max(t64[:, 2])
+    print("config 2 fp32 vs fp64: max|df|/max|f| = %.3e, max|dee|/max ee = %.3e, fp32 mass drift %.3e"
+          % (df, dee, np.max(np.abs(t32[:, 0] - t32[0, 0])) / t32[0, 0]))
+    assert df < 2e-4 and dee < 2e-4
+    assert np.max(np.abs(t64[:, 0] - t64[0, 0])) <= 1e-13 * t64[0, 0]

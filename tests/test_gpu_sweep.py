@@ -69,7 +69,8 @@ def test_sweep_3p3_every_direction(oracle, o, dtype):
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_config4_reduced_twin_all_sweeps(oracle, dtype):
     """Config 4 recipe (uniform f from the counter generator, per-cell shifts) with every n_d
-    divided by 8, 3 sweeps per direction, full element-wise parity."""
+    divided by 8 and the full schedule of BASELINE.json configs[3]: 50 sweeps per direction
+    (200 in all), element-wise parity after each direction."""
     cfg = W.CONFIG4.scaled((16, 16, 8, 8))
     s = make_solver(cfg, dtype)
     s.fill_uniform(W.SEED, W.TAG_F)
@@ -78,7 +79,7 @@ def test_config4_reduced_twin_all_sweeps(oracle, dtype):
     ref = f_host.copy()
     for dim in range(4):
         sigma = W.config4_shifts(cfg, dim)
-        for _ in range(3):
+        for _ in range(cfg.extra["sweeps_per_direction"]):
             s.translate(dim, sigma)
             oracle.translate(ref, cfg.N, cfg.order, dim, sigma, dep_of(cfg.dx, dim))
         assert rel_err(s.get_f(), ref) <= TOL[dtype], dim
