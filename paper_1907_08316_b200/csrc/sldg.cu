@@ -603,7 +603,7 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
         const size_t slot = (slab_bytes + 127) & ~(size_t)127;
         const long planes = midN * outer2;           // midN == 1 for (0, 1)
         const char *e = getenv("SLDG_NO_PLANE_PAIR");
-        if (c->use_tma && !(e && e[0] == '1') && k1 == 0 && k2 == 1 && slab_bytes % 16 == 0 && 3 * slot <= 96 * 1024 &&
+        if (c->use_tma && !(e && e[0] == '1') && k1 == 0 && k2 == 1 && slab_bytes % 16 == 0 && 4 * slot <= 96 * 1024 &&
             n1 <= 256 && n2 >= 3 && planes < (1L << 31)) {
             static bool attr_set = false;
             if (!attr_set) {
@@ -611,7 +611,7 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
                 attr_set = true;
             }
             int blk = (int)(cdiv(n1, 32) * 32);
-            sweep_xpair_plane_kernel<T, O><<<(unsigned)planes, blk, 3 * slot, c->stream>>>(
+            sweep_xpair_plane_kernel<T, O><<<(unsigned)planes, blk, 4 * slot, c->stream>>>(
                 in, out, n1, n2, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2, (const T *)c->d_ab2, count2,
                 qd2, qm2);
             LAUNCH_CHECK(c);
@@ -683,14 +683,14 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
         const size_t slab_bytes = (size_t)O * n2 * O * n1 * O * sizeof(T);
         const size_t slot = (slab_bytes + 127) & ~(size_t)127;
         if (c->use_tma && k1 == 0 && k2 == 1 && k3 == 2 && c->dx == 3 && slab_bytes % 16 == 0 &&
-            3 * slot <= 200 * 1024 && (long)n1 * n2 <= 512 && outer3 < (1L << 31)) {
+            4 * slot <= 200 * 1024 && (long)n1 * n2 <= 512 && outer3 < (1L << 31)) {
             static bool attr_set = false;
             if (!attr_set) {
                 cudaFuncSetAttribute(sweep_xtriple_plane_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
                 attr_set = true;
             }
             int block = (int)(cdiv((long)n1 * n2, 32) * 32);
-            sweep_xtriple_plane_kernel<T, O><<<(unsigned)outer3, block, 3 * slot, c->stream>>>(
+            sweep_xtriple_plane_kernel<T, O><<<(unsigned)outer3, block, 4 * slot, c->stream>>>(
                 in, out, n1, n2, n3, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2,
                 qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
             LAUNCH_CHECK(c);
