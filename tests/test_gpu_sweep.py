@@ -342,3 +342,22 @@ def test_no_write_outside_the_f_buffers(dtype):
             assert bool((b[:G] == -777.0).all()) and bool((b[G + n:] == -777.0).all()), (cells, o)
         assert bool(torch.isfinite(s.current()).all())
         s.close()
+
+
+def test_create_destroy_does_not_leak_device_memory():
+    import torch
+    cfg = W.Config("leak", 2, 2, (8, 8, 8, 8), 3, (0.0,) * 4, (1.0,) * 4, dt=0.1)
+    def cycle():
+        s = make_solver(cfg, "f64")
+        s.fill_uniform(1, 0)
+        s.step(0.1); s.step(0.1); s.step(0.1)        # includes a captured graph
+        s.diagnostics(); s.moments()
+        s.close()
+    cycle()
+    torch.cuda.synchronize(); torch.cuda.empty_cache()
+    free0, _ = torch.cuda.mem_get_info()
+    for _ in range(40):
+        cycle()
+    torch.cuda.synchronize(); torch.cuda.empty_cache()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free0 - free1 < 8 * 1024 * 1024, (free0, free1)
