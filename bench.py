@@ -134,21 +134,26 @@ def oracle_step_factory(cfg, dtype):
     shifts = [W.config4_shifts(cfg, d) for d in range(D)]
     deps = [[cfg.dx + d] if d < cfg.dx else list(range(cfg.dx)) for d in range(D)]
 
+    per_dim = {d: 0.0 for d in range(D)}      # seconds spent in the sweeps of each direction (all steps)
+
     def step():
         t_sweeps = 0.0
         for d in range(cfg.dx):
             t0 = time.perf_counter()
             O.translate(f, cfg.N, cfg.order, d, shifts[d], deps[d])
-            t_sweeps += time.perf_counter() - t0
+            dt_ = time.perf_counter() - t0
+            t_sweeps += dt_; per_dim[d] += dt_
         rho = g.rho(f)
         g.poisson_E(rho)
         for d in range(cfg.dx, D):
             t0 = time.perf_counter()
             O.translate(f, cfg.N, cfg.order, d, shifts[d], deps[d])
-            t_sweeps += time.perf_counter() - t0
+            dt_ = time.perf_counter() - t0
+            t_sweeps += dt_; per_dim[d] += dt_
         g.diagnostics(f)
         return t_sweeps
 
+    step.per_dim = per_dim
     return step, O.num_threads()
 
 
@@ -458,6 +463,7 @@ def run_ours(args):
         line["cpu_baseline"] = {
             "value": 2.0 * ocfg.ndof * es * D * nrep / t_sw / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
             "dof_updates_per_s": ocfg.ndof * D * nrep / t_sw,
+            "per_direction_gbs": {"dim%d" % d: 2.0 * ocfg.ndof * es * nrep / t / 1e9 for d, t in ostep.per_dim.items()},
             "sample": "%d bench step(s) of the config-4 recipe on reduced twin cells=%s (%.2e DOF)" % (nrep, ocfg.cells, ocfg.ndof)}
 
     if rank == 0:
