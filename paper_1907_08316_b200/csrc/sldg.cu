@@ -620,6 +620,33 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
             return SLDG_OK;
         }
     }
+    // v_a v_b at o >= 3: TMA-tile staged kernel for |shift| < 1 (lanes along inner1, per-cell tensor boxes);
+    // at o <= 2 the register kernel below is as fast
+    {
+        const char *e = getenv("SLDG_TILE_PAIR");        // 0 = never, 1 = also at o <= 2
+        const bool want = e ? (e[0] == '1') : (O >= 3);
+        const long blocks = (inner1 / 32) * (n1 / 4) * outer2;
+        if (c->use_tma && want && !(e && e[0] == '0') && k1 >= c->dx && midN == 1 && inner1 % 32 == 0 && n1 % 4 == 0 &&
+            n1 >= 4 && n2 >= 3 && inner1 < (1L << 31) && outer2 < (1L << 31) && blocks < (1L << 31)) {
+            CUtensorMap tmap;
+            if (make_tensor_map_4d(&tmap, in, sizeof(T) == 8, (uint64_t)inner1, (uint64_t)n1 * O, (uint64_t)n2 * O,
+                                   (uint64_t)outer2, 32, O, O)) {
+                const size_t smem = (size_t)3 * 6 * O * O * 32 * sizeof(T);
+                static bool attr_set = false;
+                if (!attr_set) {
+                    cudaFuncSetAttribute(sweep_vpair_tile_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+                    attr_set = true;
+                }
+                sweep_vpair_tile_kernel<T, O><<<(unsigned)blocks, 128, smem, c->stream>>>(
+                    tmap, in, out, inner1, n1, n2, outer2, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2,
+                    (const T *)c->d_ab2, count2, qd2, qm2);
+                LAUNCH_CHECK(c);
+                c->cur ^= 1;
+                c->have_rho = false;
+                return SLDG_OK;
+            }
+        }
+    }
     // (the vectorised-cell variant VEC1 helps the triple kernel but measured slower for the pair
     //  kernel at config 3: 0.906 vs 0.704 ms, so the pair always uses scalar accesses)
     sweep_pair_kernel<T, O, false><<<(unsigned)cdiv(threads, 128), 128, 0, c->stream>>>(

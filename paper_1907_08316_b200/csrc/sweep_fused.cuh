@@ -619,3 +619,171 @@ sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, 
 }
 
 }  // namespace sldg
+
+namespace sldg {
+
+// ------------------------------------------------------------------------------------------
+// v_a v_b pair STAGED BY TMA TENSOR TILES, for the physical regime |shift| < 1 cell in both
+// dimensions (every lane's cell offsets m1 in {0, n1-1}, m2 in {0, n2-1}; checked per block).
+// f viewed as [outer2][N_k2][N_k1][inner1].  A block owns W = 32 inner1 columns (lanes) x C1 = 4
+// k1-cells and walks the k2 line.  Per k2-cell it stages the C1 + 2 k1-cells c1_0-1 .. c1_0+C1 -- BOTH
+// neighbours, so a lane may look left (m1 = n1-1) or right (m1 = 0) independently of the others
+// (the field changes sign every N_1/2 columns of the flattened x index) -- as one TMA box
+// [O][O][W] per k1-cell into a ring; stage j holds k2-cell j-1, a lane with m2 = n2-1 consumes it
+// at its local step j, a lane with m2 = 0 one iteration later.  Thread (col, t1) keeps its O x O
+// window along k2; the first swept cell closes the periodic line.  No raw-value registers, loads
+// asynchronous and shared by the block.  A block that sees any other offset reads its raw values
+// straight from global memory (same arithmetic).
+// ------------------------------------------------------------------------------------------
+template <typename T, int O>
+__global__ void __launch_bounds__(128)
+sweep_vpair_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__restrict__ in, T *__restrict__ out,
+                        long inner1, int n1, int n2, long outer2,
+                        const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
+                        const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2) {
+    constexpr int W = 32, C1 = 4, NS = 3;
+    constexpr int CELL = O * O * W;                          // elements of one (k2-cell, k1-cell) box
+    constexpr int STAGE = (C1 + 2) * CELL;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t full[NS];
+    T *ring = reinterpret_cast<T *>(smem_raw);
+
+    const long tiles_x = inner1 / W;
+    const int groups1 = n1 / C1;
+    long b = blockIdx.x;
+    const int g1 = (int)(b % groups1); b /= groups1;
+    const long tx = b % tiles_x;
+    const long oo2 = b / tiles_x;
+    const int tid = threadIdx.x, col = tid % W, t1 = tid / W;
+    const int c1 = g1 * C1 + t1;
+    const long ii = tx * W + col;
+    const long s1 = inner1, s2 = (long)n1 * O * inner1;      // element strides of k1 / k2 nodes
+    const long plane = oo2 * (long)n2 * O * s2 + ii;
+    const long lin0 = plane + (long)c1 * O * s1;
+    const long q1 = (lin0 / qdiv1) % qmod1, q2 = (lin0 / qdiv2) % qmod2;
+
+    T A1[O * O], B1[O * O], A2[O * O], B2[O * O];
+#pragma unroll
+    for (int e = 0; e < O * O; ++e) {
+        A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1];
+        A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
+    }
+    const int m1 = mtab1[q1], m2 = mtab2[q2];
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+    }
+    const bool small = __syncthreads_and((m1 == 0 || m1 == n1 - 1) && (m2 == 0 || m2 == n2 - 1)) != 0;
+
+    int sa = c1 + m1; if (sa >= n1) sa -= n1;                // global path: this thread's k1 source cells
+    int sb = sa + 1; if (sb == n1) sb = 0;
+    const int la = t1 + (m1 == 0 ? 1 : 0);                   // staged path: block-local index of source cell i*
+    const int late = (m2 == 0) ? 1 : 0;                      // staged path: consumes stage j at local step j - late
+
+    auto issue = [&](int j) {                                // stage j <-> k2-cell (j - 1) mod n2
+        int cell2 = j - 1;
+        if (cell2 < 0) cell2 += n2;
+        if (cell2 >= n2) cell2 -= n2;
+        const int slot = j % NS;
+        mbar_expect_tx(&full[slot], (uint32_t)(STAGE * sizeof(T)));
+        const uint64_t pol = policy_evict_first();
+#pragma unroll
+        for (int cc = 0; cc < C1 + 2; ++cc) {
+            int cell1 = g1 * C1 - 1 + cc;
+            if (cell1 < 0) cell1 += n1;
+            if (cell1 >= n1) cell1 -= n1;
+            tma_load_4d_hint(ring + (size_t)slot * STAGE + (size_t)cc * CELL, &tmap, (int)(tx * W), cell1 * O, cell2 * O,
+                             (int)oo2, &full[slot], pol);
+        }
+    };
+    // k1-swept values of this thread's cell: from stage slot (staged) ...
+    auto k1_staged = [&](int slot, T (&w)[O][O]) {
+        const T *st = ring + (size_t)slot * STAGE + col;
+#pragma unroll
+        for (int l2 = 0; l2 < O; ++l2) {
+            T r0[O], r1[O];
+#pragma unroll
+            for (int l = 0; l < O; ++l) {
+                r0[l] = st[((la * O + l2) * O + l) * W];
+                r1[l] = st[(((la + 1) * O + l2) * O + l) * W];
+            }
+#pragma unroll
+            for (int j1 = 0; j1 < O; ++j1) w[l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+        }
+    };
+    // ... or from global memory for source k2-cell `cell2`
+    auto k1_global = [&](int cell2, T (&w)[O][O]) {
+#pragma unroll
+        for (int l2 = 0; l2 < O; ++l2) {
+            const T *row = in + plane + ((long)cell2 * O + l2) * s2;
+            T r0[O], r1[O];
+#pragma unroll
+            for (int l = 0; l < O; ++l) {
+                r0[l] = row[((long)sa * O + l) * s1];
+                r1[l] = row[((long)sb * O + l) * s1];
+            }
+#pragma unroll
+            for (int j1 = 0; j1 < O; ++j1) w[l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+        }
+    };
+    auto emit = [&](int i2, const T (&w0)[O][O], const T (&w1)[O][O]) {
+        T *dst = out + lin0 + (long)i2 * O * s2;
+#pragma unroll
+        for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+            for (int j1 = 0; j1 < O; ++j1) {
+                T a0[O], a1[O];
+#pragma unroll
+                for (int l = 0; l < O; ++l) { a0[l] = w0[l][j1]; a1[l] = w1[l][j1]; }
+                __stcs(dst + (long)j2 * s2 + (long)j1 * s1, chain<T, O>(A2, B2, j2, a0, a1));
+            }
+    };
+    auto copy = [&](T (&d)[O][O], const T (&s)[O][O]) {
+#pragma unroll
+        for (int a = 0; a < O; ++a)
+#pragma unroll
+            for (int c = 0; c < O; ++c) d[a][c] = s[a][c];
+    };
+
+    T wfirst[O][O], w0[O][O], w1[O][O];
+    if (small) {
+        if (tid == 0)
+            for (int j = 0; j < NS && j <= n2; ++j) issue(j);
+        for (int j = 0; j <= n2 + 1; ++j) {
+            const int t = j - late;                          // this thread's local step
+            if (j <= n2) {
+                mbar_wait(&full[j % NS], (uint32_t)((j / NS) & 1));
+                if (t == 0) {
+                    k1_staged(j % NS, wfirst);
+                    copy(w0, wfirst);
+                } else if (t >= 1 && t <= n2 - 1) {
+                    k1_staged(j % NS, w1);
+                    emit(t - 1, w0, w1);
+                    copy(w0, w1);
+                }
+            }
+            if (t == n2) emit(n2 - 1, w0, wfirst);           // closes the periodic line
+            if (j <= n2) {
+                __syncthreads();                             // everyone is done with this slot
+                if (tid == 0 && j + NS <= n2) issue(j + NS);
+            }
+        }
+    } else {
+        for (int t = 0; t <= n2; ++t) {
+            int cell2 = m2 + t;
+            if (cell2 >= n2) cell2 -= n2;
+            if (t == 0) {
+                k1_global(cell2, wfirst);
+                copy(w0, wfirst);
+            } else if (t <= n2 - 1) {
+                k1_global(cell2, w1);
+                emit(t - 1, w0, w1);
+                copy(w0, w1);
+            } else {
+                emit(n2 - 1, w0, wfirst);
+            }
+        }
+    }
+}
+
+}  // namespace sldg

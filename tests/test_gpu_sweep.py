@@ -361,3 +361,43 @@ def test_create_destroy_does_not_leak_device_memory():
     torch.cuda.synchronize(); torch.cuda.empty_cache()
     free1, _ = torch.cuda.mem_get_info()
     assert free0 - free1 < 8 * 1024 * 1024, (free0, free1)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("o", [1, 2, 3, 4])
+@pytest.mark.parametrize("kind", ["small-mixed-sign", "small-one-sign", "some-large"])
+def test_tile_staged_v_pair(oracle, o, dtype, kind, monkeypatch):
+    """The TMA-tile staged v-pair (both k1-neighbours staged; lanes may look left or right, early or
+    late, independently) and its per-block fallback for offsets outside {0, n-1}: bitwise equal to the
+    two single sweeps and within tolerance of the oracle."""
+    import torch
+    monkeypatch.setenv("SLDG_TILE_PAIR", "1")              # also at o <= 2
+    cfg = W.Config("tile", 2, 2, (16, 4, 8, 5), o, (0.0,) * 4, (16.0, 4.0, 8.0, 5.0))
+    assert cfg.X % 32 == 0
+    rng = np.random.default_rng(1000 + o)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
+    x = np.arange(cfg.X)
+    if kind == "small-mixed-sign":
+        sig = [0.4 * np.sin(2 * np.pi * x / 23.0), 0.7 * np.cos(2 * np.pi * x / 41.0)]
+    elif kind == "small-one-sign":
+        sig = [0.2 + 0.1 * np.sin(x), -0.5 + 0.3 * np.cos(x)]
+    else:
+        sig = [0.4 * np.sin(2 * np.pi * x / 23.0), 0.7 * np.cos(2 * np.pi * x / 41.0)]
+        sig[0][40:44] = 2.3                                  # one tile with offsets outside {0, n-1}
+        sig[1][cfg.X - 7] = -1.7
+    a = make_solver(cfg, dtype)
+    a.set_initial(f0)
+    a.translate_pair(2, torch.from_numpy(sig[0]).cuda(), 3, torch.from_numpy(sig[1]).cuda())
+    fused = a.get_f()
+    a.close()
+    b = make_solver(cfg, dtype)
+    b.set_initial(f0)
+    b.translate(2, sig[0])
+    b.translate(3, sig[1])
+    seq = b.get_f()
+    b.close()
+    assert np.array_equal(fused, seq)
+    ref = f0.copy()
+    oracle.translate(ref, cfg.N, cfg.order, 2, sig[0], [0, 1])
+    oracle.translate(ref, cfg.N, cfg.order, 3, sig[1], [0, 1])
+    assert rel_err(fused, ref) <= TOL[dtype]
