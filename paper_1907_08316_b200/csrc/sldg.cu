@@ -726,6 +726,31 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
             return SLDG_OK;
         }
     }
+    // v_a v_b v_c in the physical regime |shift| < 1: TMA-tile staged kernel
+    {
+        const char *e = getenv("SLDG_NO_TILE_TRIPLE");
+        const long blocks = (inner1 / 32) * (n1 / 4) * (n2 / 4) * outer3;
+        if (c->use_tma && !(e && e[0] == '1') && k1 >= c->dx && mid12 == 1 && mid23 == 1 && inner1 % 32 == 0 &&
+            n1 % 4 == 0 && n2 % 4 == 0 && n3 >= 3 && inner1 < (1L << 31) && blocks < (1L << 31)) {
+            CUtensorMap tmap;
+            if (make_tensor_map_5d(&tmap, in, sizeof(T) == 8, (uint64_t)inner1, (uint64_t)n1 * O, (uint64_t)n2 * O,
+                                   (uint64_t)n3 * O, (uint64_t)outer3, 32, O, O, O)) {
+                const size_t smem = (size_t)2 * 36 * O * O * O * 32 * sizeof(T);
+                static bool attr_set = false;
+                if (!attr_set) {
+                    cudaFuncSetAttribute(sweep_vtriple_tile_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+                    attr_set = true;
+                }
+                sweep_vtriple_tile_kernel<T, O><<<(unsigned)blocks, 512, smem, c->stream>>>(
+                    tmap, in, out, inner1, n1, n2, n3, outer3, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1],
+                    (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+                LAUNCH_CHECK(c);
+                c->cur ^= 1;
+                c->have_rho = false;
+                return SLDG_OK;
+            }
+        }
+    }
     int chunk = 32;
     while (inner1 % chunk) chunk /= 2;
     long threads = inner1 * n1 * mid12 * n2 * mid23 * outer3;

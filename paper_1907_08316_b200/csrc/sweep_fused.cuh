@@ -679,16 +679,20 @@ sweep_vpair_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__res
     int sb = sa + 1; if (sb == n1) sb = 0;
     const int la = t1 + (m1 == 0 ? 1 : 0);                   // staged path: block-local index of source cell i*
     const int late = (m2 == 0) ? 1 : 0;                      // staged path: consumes stage j at local step j - late
+    // a tile without a sign change of the field needs only one neighbour cell (5 boxes instead of 6)
+    const bool needL1 = __syncthreads_or(m1 != 0) != 0, needR1 = __syncthreads_or(m1 == 0) != 0;
+    const int nboxes = C1 + (needL1 ? 1 : 0) + (needR1 ? 1 : 0);
 
     auto issue = [&](int j) {                                // stage j <-> k2-cell (j - 1) mod n2
         int cell2 = j - 1;
         if (cell2 < 0) cell2 += n2;
         if (cell2 >= n2) cell2 -= n2;
         const int slot = j % NS;
-        mbar_expect_tx(&full[slot], (uint32_t)(STAGE * sizeof(T)));
+        mbar_expect_tx(&full[slot], (uint32_t)(nboxes * CELL * sizeof(T)));
         const uint64_t pol = policy_evict_first();
 #pragma unroll
         for (int cc = 0; cc < C1 + 2; ++cc) {
+            if ((cc == 0 && !needL1) || (cc == C1 + 1 && !needR1)) continue;
             int cell1 = g1 * C1 - 1 + cc;
             if (cell1 < 0) cell1 += n1;
             if (cell1 >= n1) cell1 -= n1;
@@ -781,6 +785,211 @@ sweep_vpair_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__res
                 copy(w0, w1);
             } else {
                 emit(n2 - 1, w0, wfirst);
+            }
+        }
+    }
+}
+
+}  // namespace sldg
+
+namespace sldg {
+
+// ------------------------------------------------------------------------------------------
+// v_a v_b v_c triple STAGED BY TMA TENSOR TILES for |shift| < 1 cell in all three dimensions (the
+// 3+3 D step), one level up from sweep_vpair_tile_kernel.  f viewed as
+// [outer3][N_k3][N_k2][N_k1][inner1].  A block owns W = 32 inner1 columns (lanes) x C1 = 4 k1-cells
+// x C2 = 4 k2-cells (512 threads) and walks the k3 line; per k3-cell it stages the (C1+2) x (C2+2)
+// cell pairs (both neighbours in k1 and in k2) as one 5-D TMA box [O][O][O][W] each into a 2-deep
+// ring.  Thread (col, t1, t2) reads its 2 x 2 source cells with its own left/right choices, keeps
+// its O^3 window along k3, consumes stage j at local step j (m3 = n3-1) or j-1 (m3 = 0).
+// Bit-identical to the three sweeps; per-block fallback to direct global reads otherwise.
+// ------------------------------------------------------------------------------------------
+template <typename T, int O>
+__global__ void __launch_bounds__(512, 1)
+sweep_vtriple_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__restrict__ in, T *__restrict__ out,
+                          long inner1, int n1, int n2, int n3, long outer3,
+                          const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
+                          const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2,
+                          const int *__restrict__ mtab3, const T *__restrict__ ab3, long count3, long qdiv3, long qmod3) {
+    constexpr int W = 32, C1 = 4, C2 = 4, NS = 2;
+    constexpr int CELL = O * O * O * W;                      // elements of one (k3, k2, k1)-cell box
+    constexpr int STAGE = (C1 + 2) * (C2 + 2) * CELL;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t full[NS];
+    T *ring = reinterpret_cast<T *>(smem_raw);
+
+    const long tiles_x = inner1 / W;
+    const int groups1 = n1 / C1, groups2 = n2 / C2;
+    long b = blockIdx.x;
+    const int g1 = (int)(b % groups1); b /= groups1;
+    const int g2 = (int)(b % groups2); b /= groups2;
+    const long tx = b % tiles_x;
+    const long oo3 = b / tiles_x;
+    const int tid = threadIdx.x, col = tid % W, t1 = (tid / W) % C1, t2 = tid / (W * C1);
+    const int c1 = g1 * C1 + t1, c2 = g2 * C2 + t2;
+    const long ii = tx * W + col;
+    const long s1 = inner1, s2 = (long)n1 * O * s1, s3 = (long)n2 * O * s2;
+    const long plane = oo3 * (long)n3 * O * s3 + ii;
+    const long lin0 = plane + (long)c1 * O * s1 + (long)c2 * O * s2;
+    const long q1 = (lin0 / qdiv1) % qmod1, q2 = (lin0 / qdiv2) % qmod2, q3 = (lin0 / qdiv3) % qmod3;
+
+    T A1[O * O], B1[O * O], A2[O * O], B2[O * O], A3[O * O], B3[O * O];
+#pragma unroll
+    for (int e = 0; e < O * O; ++e) {
+        A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1];
+        A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
+        A3[e] = ab3[(long)e * count3 + q3]; B3[e] = ab3[(long)(O * O + e) * count3 + q3];
+    }
+    const int m1 = mtab1[q1], m2 = mtab2[q2], m3 = mtab3[q3];
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+    }
+    const bool small = __syncthreads_and((m1 == 0 || m1 == n1 - 1) && (m2 == 0 || m2 == n2 - 1) &&
+                                         (m3 == 0 || m3 == n3 - 1)) != 0;
+    int sa1 = c1 + m1; if (sa1 >= n1) sa1 -= n1;             // global path
+    int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
+    int sa2 = c2 + m2; if (sa2 >= n2) sa2 -= n2;
+    int sb2 = sa2 + 1; if (sb2 == n2) sb2 = 0;
+    const int la = t1 + (m1 == 0 ? 1 : 0), lb = t2 + (m2 == 0 ? 1 : 0);   // staged path: local source cells
+    const int late = (m3 == 0) ? 1 : 0;
+    // which neighbour columns / rows of cells the block really needs (a tile without a sign change of
+    // the field needs only one side: 25 instead of 36 cell pairs per 16 owned)
+    const bool needL1 = __syncthreads_or(m1 != 0) != 0, needR1 = __syncthreads_or(m1 == 0) != 0;
+    const bool needL2 = __syncthreads_or(m2 != 0) != 0, needR2 = __syncthreads_or(m2 == 0) != 0;
+    const int nboxes = (C1 + (needL1 ? 1 : 0) + (needR1 ? 1 : 0)) * (C2 + (needL2 ? 1 : 0) + (needR2 ? 1 : 0));
+
+    auto issue = [&](int j) {                                // stage j <-> k3-cell (j - 1) mod n3; all threads call
+        int cell3 = j - 1;
+        if (cell3 < 0) cell3 += n3;
+        if (cell3 >= n3) cell3 -= n3;
+        const int slot = j % NS;
+        if (tid == 0) mbar_expect_tx(&full[slot], (uint32_t)(nboxes * CELL * sizeof(T)));
+        const int ca = tid % (C1 + 2), cb = tid / (C1 + 2);
+        if (tid < (C1 + 2) * (C2 + 2) && (ca > 0 || needL1) && (ca < C1 + 1 || needR1) && (cb > 0 || needL2) &&
+            (cb < C2 + 1 || needR2)) {
+            int cell1 = g1 * C1 - 1 + ca;
+            if (cell1 < 0) cell1 += n1;
+            if (cell1 >= n1) cell1 -= n1;
+            int cell2 = g2 * C2 - 1 + cb;
+            if (cell2 < 0) cell2 += n2;
+            if (cell2 >= n2) cell2 -= n2;
+            tma_load_5d_hint(ring + (size_t)slot * STAGE + (size_t)tid * CELL, &tmap, (int)(tx * W), cell1 * O, cell2 * O,
+                             cell3 * O, (int)oo3, &full[slot], policy_evict_first());
+        }
+    };
+    auto k12_staged = [&](int slot, T (&w)[O][O][O]) {
+        const T *st = ring + (size_t)slot * STAGE + col;
+#pragma unroll
+        for (int l3 = 0; l3 < O; ++l3) {
+            T tk[2][O][O];
+#pragma unroll
+            for (int e2 = 0; e2 < 2; ++e2)
+#pragma unroll
+                for (int l2 = 0; l2 < O; ++l2) {
+                    const T *p0 = st + (size_t)((lb + e2) * (C1 + 2) + la) * CELL + ((l3 * O + l2) * O) * W;
+                    T r0[O], r1[O];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) { r0[l] = p0[l * W]; r1[l] = p0[CELL + l * W]; }
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) tk[e2][l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+                }
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a0[O], a1[O];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) { a0[l] = tk[0][l][j1]; a1[l] = tk[1][l][j1]; }
+                    w[l3][j2][j1] = chain<T, O>(A2, B2, j2, a0, a1);
+                }
+        }
+    };
+    auto k12_global = [&](int cell3, T (&w)[O][O][O]) {
+#pragma unroll
+        for (int l3 = 0; l3 < O; ++l3) {
+            const T *row = in + plane + ((long)cell3 * O + l3) * s3;
+            T tk[2][O][O];
+#pragma unroll
+            for (int e2 = 0; e2 < 2; ++e2)
+#pragma unroll
+                for (int l2 = 0; l2 < O; ++l2) {
+                    const T *p = row + ((long)(e2 ? sb2 : sa2) * O + l2) * s2;
+                    T r0[O], r1[O];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) { r0[l] = p[((long)sa1 * O + l) * s1]; r1[l] = p[((long)sb1 * O + l) * s1]; }
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) tk[e2][l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+                }
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a0[O], a1[O];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) { a0[l] = tk[0][l][j1]; a1[l] = tk[1][l][j1]; }
+                    w[l3][j2][j1] = chain<T, O>(A2, B2, j2, a0, a1);
+                }
+        }
+    };
+    auto emit = [&](int i3, const T (&w0)[O][O][O], const T (&w1)[O][O][O]) {
+        T *dst = out + lin0 + (long)i3 * O * s3;
+#pragma unroll
+        for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a0[O], a1[O];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) { a0[l] = w0[l][j2][j1]; a1[l] = w1[l][j2][j1]; }
+                    __stcs(dst + (long)j3 * s3 + (long)j2 * s2 + (long)j1 * s1, chain<T, O>(A3, B3, j3, a0, a1));
+                }
+    };
+    auto copy = [&](T (&d)[O][O][O], const T (&s)[O][O][O]) {
+#pragma unroll
+        for (int a = 0; a < O; ++a)
+#pragma unroll
+            for (int c = 0; c < O; ++c)
+#pragma unroll
+                for (int e = 0; e < O; ++e) d[a][c][e] = s[a][c][e];
+    };
+
+    T wfirst[O][O][O], w0[O][O][O], w1[O][O][O];
+    if (small) {
+        for (int j = 0; j < NS && j <= n3; ++j) issue(j);
+        for (int j = 0; j <= n3 + 1; ++j) {
+            const int t = j - late;
+            if (j <= n3) {
+                mbar_wait(&full[j % NS], (uint32_t)((j / NS) & 1));
+                if (t == 0) {
+                    k12_staged(j % NS, wfirst);
+                    copy(w0, wfirst);
+                } else if (t >= 1 && t <= n3 - 1) {
+                    k12_staged(j % NS, w1);
+                    emit(t - 1, w0, w1);
+                    copy(w0, w1);
+                }
+            }
+            if (t == n3) emit(n3 - 1, w0, wfirst);
+            if (j <= n3) {
+                __syncthreads();
+                if (j + NS <= n3) issue(j + NS);
+            }
+        }
+    } else {
+        for (int t = 0; t <= n3; ++t) {
+            int cell3 = m3 + t;
+            if (cell3 >= n3) cell3 -= n3;
+            if (t == 0) {
+                k12_global(cell3, wfirst);
+                copy(w0, wfirst);
+            } else if (t <= n3 - 1) {
+                k12_global(cell3, w1);
+                emit(t - 1, w0, w1);
+                copy(w0, w1);
+            } else {
+                emit(n3 - 1, w0, wfirst);
             }
         }
     }

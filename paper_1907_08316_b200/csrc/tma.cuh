@@ -104,6 +104,15 @@ __device__ __forceinline__ void tma_load_4d_hint(void *smem_dst, const CUtensorM
         : "memory");
 }
 
+__device__ __forceinline__ void tma_load_5d_hint(void *smem_dst, const CUtensorMap *tmap, int c0, int c1, int c2, int c3,
+                                                 int c4, uint64_t *bar, uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, "
+        "{%2, %3, %4, %5, %6}], [%7], %8;" ::"r"(smem_u32(smem_dst)),
+        "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(bar)), "l"(pol)
+        : "memory");
+}
+
 // L2 prefetch of a contiguous span (multiple of 16 bytes, 16-byte aligned) by the copy engine
 __device__ __forceinline__ void bulk_prefetch_l2(const void *gmem, uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem), "r"(bytes) : "memory");
@@ -155,6 +164,23 @@ inline bool make_tensor_map_4d(CUtensorMap *map, const void *base, bool is_f64, 
     cuuint32_t box[4] = {b0, b1, b2, 1};
     cuuint32_t estr[4] = {1, 1, 1, 1};
     CUresult r = enc(map, is_f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4,
+                     const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+// f viewed as [d4][d3][d2][d1][d0] (d0 fastest); box = [1][b3][b2][b1][b0]
+inline bool make_tensor_map_5d(CUtensorMap *map, const void *base, bool is_f64, uint64_t d0, uint64_t d1, uint64_t d2,
+                               uint64_t d3, uint64_t d4, uint32_t b0, uint32_t b1, uint32_t b2, uint32_t b3) {
+    tensor_map_encode_fn enc = get_tensor_map_encoder();
+    if (!enc) return false;
+    const uint64_t es = is_f64 ? 8 : 4;
+    cuuint64_t dims[5] = {d0, d1, d2, d3, d4};
+    cuuint64_t strides[4] = {d0 * es, d0 * d1 * es, d0 * d1 * d2 * es, d0 * d1 * d2 * d3 * es};
+    cuuint32_t box[5] = {b0, b1, b2, b3, 1};
+    cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    CUresult r = enc(map, is_f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5,
                      const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                      CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);

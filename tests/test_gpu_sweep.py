@@ -401,3 +401,41 @@ def test_tile_staged_v_pair(oracle, o, dtype, kind, monkeypatch):
     oracle.translate(ref, cfg.N, cfg.order, 2, sig[0], [0, 1])
     oracle.translate(ref, cfg.N, cfg.order, 3, sig[1], [0, 1])
     assert rel_err(fused, ref) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("o", [1, 2])
+@pytest.mark.parametrize("kind", ["small-mixed-sign", "small-one-sign", "some-large"])
+def test_tile_staged_v_triple(oracle, o, dtype, kind):
+    """The TMA-tile staged v-triple (both neighbours staged in v_1 and v_2, early/late in v_3) and its
+    per-block fallback: bitwise equal to the three single sweeps, within tolerance of the oracle."""
+    import torch
+    cfg = W.Config("tile3", 3, 3, (4, 4, 2, 4, 8, 5), o, (0.0,) * 6, (4.0, 4.0, 2.0, 4.0, 8.0, 5.0))
+    assert cfg.X % 32 == 0
+    rng = np.random.default_rng(2000 + o)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
+    x = np.arange(cfg.X)
+    if kind == "small-one-sign":
+        sig = [0.2 + 0.1 * np.sin(x), -0.5 + 0.3 * np.cos(x), 0.6 + 0.2 * np.sin(0.3 * x)]
+    else:
+        sig = [0.4 * np.sin(2 * np.pi * x / 23.0), 0.7 * np.cos(2 * np.pi * x / 41.0), 0.9 * np.sin(2 * np.pi * x / 17.0)]
+        if kind == "some-large":
+            sig[0][3:6] = 2.3
+            sig[2][cfg.X - 7] = -1.7
+    a = make_solver(cfg, dtype)
+    a.set_initial(f0)
+    a.translate_triple(3, torch.from_numpy(sig[0]).cuda(), 4, torch.from_numpy(sig[1]).cuda(),
+                       5, torch.from_numpy(sig[2]).cuda())
+    fused = a.get_f()
+    a.close()
+    b = make_solver(cfg, dtype)
+    b.set_initial(f0)
+    for k, s_ in zip((3, 4, 5), sig):
+        b.translate(k, s_)
+    seq = b.get_f()
+    b.close()
+    assert np.array_equal(fused, seq)
+    ref = f0.copy()
+    for k, s_ in zip((3, 4, 5), sig):
+        oracle.translate(ref, cfg.N, cfg.order, k, s_, [0, 1, 2])
+    assert rel_err(fused, ref) <= TOL[dtype]
