@@ -18,8 +18,12 @@
  * (R9); the Gauss-Legendre rule and the A,B quadrature are carried out in long double
  * internally and rounded ONCE to double (O7: 'rounded once' taken literally).  Every function returns 0 on success, nonzero on a bad argument.
  *
- * Pins (tests/test_oracle_pins.py): P1..P13 of S:§8(c).  Config-2 two-stream
- * growth is "parity unpinned" by the paper (its eq. (2) is a different state).
+ * Pins: P1..P13 of S:§8(c) in tests/test_oracle_pins.py, test_oracle_sweep_pins.py,
+ * test_oracle_physics_pins.py, test_oracle_moment_pins.py; the three-dimensional branches
+ * (Poisson mode decode, d_v = 3 weights, 3+3 D step), the 2+2 D Landau rate and the global sums
+ * against exact summation in tests/test_oracle_3d_pins.py; A,B against exact values (<= 1/2 ulp +
+ * 1e-18) in tests/test_oracle_ab_exact.py; ASan/UBSan in tests/test_oracle_sanitizers.py.
+ * Config-2 two-stream growth is "parity unpinned" by the paper (its eq. (2) is a different state).
  */
 #ifndef SLDG_ORACLE_H
 #define SLDG_ORACLE_H
@@ -89,7 +93,8 @@ int oracle_step_f64(double *f, int dx, int dv, const int *cells, int o,
 int oracle_step_f32(float *f, int dx, int dv, const int *cells, int o,
                     const double *lo, const double *hi, double dt);
 
-/* O6 row a-6 / R12: mass = sum W f, l2 = sqrt(sum W f^2), ee = 1/2 sum_x W_x |E|^2. */
+/* O6 row a-6 / R12: mass = sum W f, l2 = sqrt(sum W f^2) as single running sums over all N nodes in
+ * canonical order, long double accumulator rounded once; ee = 1/2 sum_x W_x |E|^2. */
 int oracle_diagnostics_f64(const double *f, int dx, int dv, const int *cells, int o,
                            const double *lo, const double *hi,
                            double *mass, double *l2, double *ee);
@@ -98,7 +103,7 @@ int oracle_diagnostics_f32(const float *f, int dx, int dv, const int *cells, int
                            double *mass, double *l2, double *ee);
 
 /* S:8(f) NEXT-4 (Fig. 15): momentum[a] = int int v_a f (a < dv) and
- * kinetic = 1/2 int int |v|^2 f by Gauss quadrature on the nodes, iterated sums (R12). */
+ * kinetic = 1/2 int int |v|^2 f by Gauss quadrature on the nodes: single running sums in long double (R12). */
 int oracle_moments_f64(const double *f, int dx, int dv, const int *cells, int o,
                        const double *lo, const double *hi, double *momentum, double *kinetic);
 int oracle_moments_f32(const float *f, int dx, int dv, const int *cells, int o,
