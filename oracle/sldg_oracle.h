@@ -76,7 +76,8 @@ int oracle_advect_f64(double *f, int dx, int dv, const int *cells, int o,
 int oracle_advect_f32(float *f, int dx, int dv, const int *cells, int o,
                       const double *lo, const double *hi, int dim, double tau, const double *E);
 
-/* O4: rho[x] = - sum_v W_v f[v][x], fp64 accumulation, v_dv outermost. */
+/* O4: rho[x] = - sum_v W_v f[v][x]: the sum over all velocity nodes in canonical order,
+ * accumulated in long double and rounded to double once (no grouping, D:O4). */
 int oracle_rho_f64(const double *f, int dx, int dv, const int *cells, int o,
                    const double *lo, const double *hi, double *rho);
 int oracle_rho_f32(const float *f, int dx, int dv, const int *cells, int o,

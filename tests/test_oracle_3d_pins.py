@@ -172,6 +172,40 @@ def test_global_sums_are_the_exact_sums_rounded(oracle, dx, dv, cells, dtype):
     assert abs(K - 0.5 * float(k)) <= 2 * ulp(abs(0.5 * float(k))) + 1e-17 * scale_m
 
 
+@pytest.mark.parametrize("dx,dv,cells,dtype", [(1, 1, (5, 300), np.float64), (2, 2, (2, 3, 20, 24), np.float64),
+                                               (1, 3, (3, 8, 6, 10), np.float32), (3, 3, (1, 2, 1, 6, 5, 7), np.float64)])
+def test_rho_is_the_exact_sum_rounded(oracle, dx, dv, cells, dtype):
+    """O4: rho[x] = -sum_v W_v f[v][x] is a sum with no order.  The oracle's long-double running sum
+    must give the exactly summed value (rational arithmetic on the same doubles) to 1 ulp -- with mixed-sign
+    terms spanning six decades, where a double running sum over the same V terms is visibly off."""
+    from fractions import Fraction as Fr
+    o = 2
+    lo = (0.0,) * dx + (-4.0, -3.0, -5.0)[:dv]
+    hi = tuple(1.0 + 0.5 * a for a in range(dx)) + (4.5, 3.5, 4.0)[:dv]
+    g = oracle.Grid(dx, dv, cells, o, lo, hi)
+    rng = np.random.default_rng(7)
+    f = (rng.uniform(-1.0, 1.0, g.ndof) * 10.0 ** rng.uniform(-6, 0, g.ndof)).astype(dtype)
+    xi, w = oracle.gauss_legendre(o)
+    Wv = np.ones(1)
+    for a in range(dv):                       # ((1 * W_1) * W_2) * W_3 per node, v_1 fastest
+        wa = np.tile(w * ((hi[dx + a] - lo[dx + a]) / cells[dx + a]), cells[dx + a])
+        Wv = (Wv[None, :] * wa[:, None]).reshape(-1)
+    V, X = Wv.size, g.X
+    fv = f.astype(np.float64).reshape(V, X)
+    rho = g.rho(f)
+    worst_naive = 0.0
+    for x in range(X):
+        exact = -sum((Fr(float(Wv[v])) * Fr(float(fv[v, x])) for v in range(V)), Fr(0))
+        scale = float(np.sum(np.abs(Wv * fv[:, x])))
+        assert abs(Fr(float(rho[x])) - exact) <= Fr(float(np.spacing(abs(float(exact))))) + Fr(scale) * Fr(1, 10 ** 18), x
+        naive = 0.0
+        for v in range(V):
+            naive += Wv[v] * fv[v, x]
+        worst_naive = max(worst_naive, abs(float(Fr(-naive) - exact)) / scale)
+    if V >= 1000:
+        assert worst_naive > 2e-17           # the double running sum really is worse (what the oracle avoids)
+
+
 # ---------------------------------------------------------------- P9 for the config-5 state (3+3 D)
 
 def test_P9_initial_field_of_the_3p3_landau_state(oracle):
