@@ -13,8 +13,25 @@
 
 namespace sldg {
 
+// Compensated accumulation (Knuth two-sum + the exact product error from one FMA): (hi, lo) carries
+// the running sum to about twice the working precision, so hi + lo is the exactly summed value rounded
+// once -- what D:O4 defines rho to be.  Used where a thread sums a whole v-line alone (one split) and
+// in the pass over the splits; the split partials of large problems are short sums already.
+__device__ __forceinline__ void two_sum_acc(double &hi, double &lo, double t) {
+    const double s = hi + t;
+    const double bb = s - hi;
+    lo += (hi - (s - bb)) + (t - bb);
+    hi = s;
+}
+__device__ __forceinline__ void comp_add_product(double &hi, double &lo, double w, double val) {
+    const double p = w * val;
+    lo += fma(w, val, -p);
+    two_sum_acc(hi, lo, p);
+}
+
 // part_rho[split][x] = sum_{v in split} W_v f[v][x];  part_s2 likewise with f^2 (if WITH_S2)
-template <typename T, int VEC, bool WITH_S2, int UB>
+// COMP: compensated accumulation of the rho sum (one-split launches: the partial IS rho).
+template <typename T, int VEC, bool WITH_S2, int UB, bool COMP = false>
 __global__ void __launch_bounds__(128)
 vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
                     const double *__restrict__ Wv, double *__restrict__ part_rho,
@@ -27,9 +44,9 @@ vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
     const long v0 = split * vps;
     long v1 = v0 + vps;
     if (v1 > V) v1 = V;
-    double acc[VEC], acc2[VEC];
+    double acc[VEC], acc2[VEC], lo[VEC];
 #pragma unroll
-    for (int e = 0; e < VEC; ++e) { acc[e] = 0.0; acc2[e] = 0.0; }
+    for (int e = 0; e < VEC; ++e) { acc[e] = 0.0; acc2[e] = 0.0; lo[e] = 0.0; }
     const T *p = f + v0 * X + x;
     long v = v0;
     for (; v + UB <= v1; v += UB) {
@@ -46,7 +63,8 @@ vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
             for (int e = 0; e < VEC; ++e) {
                 double val = (double)u[b].v[e];
                 double wv = w[b] * val;
-                acc[e] += wv;
+                if (COMP) comp_add_product(acc[e], lo[e], w[b], val);
+                else acc[e] += wv;
                 if (WITH_S2) acc2[e] = fma(wv, val, acc2[e]);
             }
         p += (long)UB * X;
@@ -58,14 +76,15 @@ vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
         for (int e = 0; e < VEC; ++e) {
             double val = (double)u.v[e];
             double wv = w * val;
-            acc[e] += wv;
+            if (COMP) comp_add_product(acc[e], lo[e], w, val);
+            else acc[e] += wv;
             if (WITH_S2) acc2[e] = fma(wv, val, acc2[e]);
         }
         p += X;
     }
 #pragma unroll
     for (int e = 0; e < VEC; ++e) {
-        part_rho[split * X + x + e] = acc[e];
+        part_rho[split * X + x + e] = COMP ? acc[e] + lo[e] : acc[e];
         if (WITH_S2) part_s2[split * X + x + e] = acc2[e];
     }
 }
@@ -82,12 +101,18 @@ vsum_final_kernel(const double *__restrict__ part_rho, const double *__restrict_
     const long x = ((long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (x >= X) return;
-    double a = 0.0, b = 0.0;
+    double a = 0.0, al = 0.0, b = 0.0;
     for (int s = lane; s < splits; s += 32) {
-        a += part_rho[(long)s * X + x];
+        two_sum_acc(a, al, part_rho[(long)s * X + x]);
         if (part_s2) b += part_s2[(long)s * X + x];
     }
-    a = warp_sum(a);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {             // fixed tree on (hi, lo) pairs
+        const double oh = __shfl_down_sync(0xffffffffu, a, off), ol = __shfl_down_sync(0xffffffffu, al, off);
+        two_sum_acc(a, al, oh);
+        al += ol;
+    }
+    a += al;
     b = warp_sum(b);
     if (lane == 0) {
         rho[x] = -a;

@@ -10,6 +10,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <unordered_map>
 #include <vector>
 
 #include "fill.cuh"
@@ -38,7 +39,22 @@ struct sldg_ctx {
     void *buf[2] = {nullptr, nullptr};
     int cur = 0;
     cudaStream_t stream = nullptr;
+    int device = 0;                    // the device the context was created on; every entry point runs there
     int sm_count = 148;
+    // dynamic shared memory opt-in (cudaFuncAttributeMaxDynamicSharedMemorySize) is per device and per
+    // kernel: remembered per CONTEXT (a context lives on one device), never in process-wide statics
+    std::unordered_map<const void *, size_t> smem_attr;
+    // tuning switches, read from the environment ONCE in sldg_create
+    struct Tune {
+        int tile_w = 0;                // SLDG_TILE_W: columns per TMA tile of the v-sweeps (0 = default)
+        bool plane_pair = true;        // SLDG_NO_PLANE_PAIR=1 -> false
+        int tile_pair = -1;            // SLDG_TILE_PAIR: -1 default (o >= 3), 0 never, 1 always
+        bool tile_triple = true;       // SLDG_NO_TILE_TRIPLE=1 -> false
+        int vt_variant = -1;           // SLDG_VTRIPLE_VARIANT: staged v-triple variant (-1 = default)
+    } tune;
+    // TMA descriptors depend only on (buffer, view), both fixed for the life of the context: encoded once
+    struct TmapSlot { CUtensorMap map; bool valid = false; int p0 = 0, p1 = 0; };
+    TmapSlot tmap3[SLDG_MAX_DIM][2], tmap4[SLDG_MAX_DIM][2], tmap5[2];
 
     // device tables
     double *d_coef = nullptr;          // A/B polynomial coefficients [2][o][o][2o]
@@ -53,6 +69,8 @@ struct sldg_ctx {
         void *ab = nullptr;            // [2 o^2][cap] of T
         double tau = 0.0;
         bool valid = false;            // m/ab hold the assembled table for `tau`
+        double pending_tau = 0.0;      // sigma was filled for this tau; valid once the sweep that assembles succeeded
+        bool pending = false;
     };
     Tab gen[3], xt[3];
     // the table set(s) the next sweep launch reads: aliases into gen[] / xt[]
@@ -124,6 +142,42 @@ int fail(sldg_ctx *c, int code, const char *fmt, ...) {
     } while (0)
 
 inline long cdiv(long a, long b) { return (a + b - 1) / b; }
+
+// Runs the enclosing entry point on the context's device, whatever device is current in the calling
+// thread, and restores the caller's device on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const sldg_ctx *c) {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device)
+            switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
+// opt in to `bytes` of dynamic shared memory for `kernel` on this context's device (once per size)
+template <typename K>
+cudaError_t ensure_smem(sldg_ctx *c, K kernel, size_t bytes) {
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    size_t &have = c->smem_attr[(const void *)kernel];
+    if (bytes <= have) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) have = bytes;
+    return e;
+}
+
+int env_int(const char *name, int dflt, int lo, int hi) {
+    const char *e = getenv(name);
+    if (!e || !e[0]) return dflt;
+    char *end = nullptr;
+    long v = strtol(e, &end, 10);
+    if (end == e || v < lo || v > hi) return dflt;       // out of range or not a number: ignored
+    return (int)v;
+}
+bool env_flag(const char *name) {
+    const char *e = getenv(name);
+    return e && e[0] == '1';
+}
 
 template <typename P>
 cudaError_t dalloc(P **p, size_t count) {
@@ -204,17 +258,34 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         if (d < dx) c->X *= c->N[d]; else c->V *= c->N[d];
     }
     gauss_legendre_01(order, c->xi, c->w);
-    {
-        const char *e = getenv("SLDG_NO_TMA");
-        c->use_tma = !(e && e[0] == '1');
-        e = getenv("SLDG_NO_FUSE");
-        c->use_fuse = !(e && e[0] == '1');
-        e = getenv("SLDG_NO_GRAPH");
-        c->use_graph = !(e && e[0] == '1') && c->ndof <= (1L << 24);
+    {   // the environment is read here and nowhere else
+        c->use_tma = !env_flag("SLDG_NO_TMA");
+        c->use_fuse = !env_flag("SLDG_NO_FUSE");
+        c->use_graph = !env_flag("SLDG_NO_GRAPH") && c->ndof <= (1L << 24);
+        c->tune.plane_pair = !env_flag("SLDG_NO_PLANE_PAIR");
+        c->tune.tile_triple = !env_flag("SLDG_NO_TILE_TRIPLE");
+        c->tune.tile_pair = env_int("SLDG_TILE_PAIR", -1, 0, 1);
+        c->tune.vt_variant = env_int("SLDG_VTRIPLE_VARIANT", -1, 0, 15);
+        // columns per tile: a power of two in [8, 128] whose row is a multiple of 16 bytes; anything else is ignored
+        int w = env_int("SLDG_TILE_W", 0, 8, 128);
+        if (w > 0 && (w & (w - 1)) == 0 && (w * (int)c->esize) % 16 == 0) c->tune.tile_w = w;
     }
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    {   // the context lives on the device that owns the caller's buffers (falls back to the current device)
+        cudaPointerAttributes pa;
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaPointerGetAttributes(&pa, f_buf0) == cudaSuccess && pa.type == cudaMemoryTypeDevice) dev = pa.device;
+        else cudaGetLastError();
+        c->device = dev;
+        cudaPointerAttributes pb;
+        if (cudaPointerGetAttributes(&pb, f_buf1) == cudaSuccess && pb.type == cudaMemoryTypeDevice && pb.device != dev) {
+            delete c;
+            return fail(nullptr, SLDG_ERR_ARG, "sldg_create: the two f buffers live on different devices");
+        }
+        cudaGetLastError();
+    }
+    DeviceGuard guard(c);
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
 
 #define CREATE_TRY(call)                                                                        \
     do {                                                                                        \
@@ -354,6 +425,7 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
 
 extern "C" int sldg_destroy(sldg_ctx *ctx) {
     if (!ctx) return SLDG_ERR_ARG;
+    DeviceGuard guard(ctx);
     cudaStreamSynchronize(ctx->stream);
     for (auto &g : ctx->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
     if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
@@ -367,6 +439,7 @@ extern "C" int sldg_destroy(sldg_ctx *ctx) {
 // ------------------------------------------------------------------------------------------
 extern "C" int sldg_set_initial(sldg_ctx *c, const void *src, int is_device) {
     if (!c || !src) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     size_t bytes = (size_t)c->ndof * c->esize;
     CUDA_TRY(c, cudaMemcpyAsync(c->buf[c->cur], src, bytes,
                                 is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
@@ -377,6 +450,7 @@ extern "C" int sldg_set_initial(sldg_ctx *c, const void *src, int is_device) {
 
 extern "C" int sldg_get_f(sldg_ctx *c, void *dst, int is_device) {
     if (!c || !dst) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     size_t bytes = (size_t)c->ndof * c->esize;
     CUDA_TRY(c, cudaMemcpyAsync(dst, c->buf[c->cur], bytes,
                                 is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
@@ -386,6 +460,7 @@ extern "C" int sldg_get_f(sldg_ctx *c, void *dst, int is_device) {
 
 extern "C" int sldg_fill_uniform(sldg_ctx *c, unsigned long long seed, unsigned tag) {
     if (!c) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     int blocks = c->sm_count * 8;
     if (c->dtype == SLDG_F64)
         fill_uniform_kernel<double><<<blocks, 256, 0, c->stream>>>((double *)c->buf[c->cur], c->ndof, seed, tag);
@@ -466,11 +541,7 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
             int chunks = (int)cdiv(lpg, R);
             size_t half = ((size_t)R * line_bytes + 127) & ~(size_t)127;
             size_t smem = 2 * half;
-            static size_t attr_set = 0;
-            if (smem > attr_set) {
-                cudaFuncSetAttribute(sweep_x1_bulk_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-                attr_set = 200 * 1024;
-            }
+            CUDA_TRY(c, ensure_smem(c, sweep_x1_bulk_kernel<T, O>, smem));
             long ncell = R * n;
             int block = ncell >= max_block ? max_block : (int)(cdiv(ncell, 32) * 32);
             if (block < 64) block = 64;
@@ -500,7 +571,7 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
         bool done = false;
         const long Nk = (long)n * O;
         int W = 512 / (int)sizeof(T);                        // 512-byte rows (64 columns in fp64): +0.5-0.9 % over 256 B at config 4
-        if (const char *ew = getenv("SLDG_TILE_W")) W = atoi(ew);   // tuning knob (columns per tile)
+        if (c->tune.tile_w) W = c->tune.tile_w;              // tuning knob (columns per tile), validated in sldg_create
         int nbox = (int)cdiv(Nk, 256);
         int box_rows = (int)cdiv(Nk, nbox);
         while (W > 8 && (size_t)nbox * box_rows * W * sizeof(T) > 100 * 1024) W /= 2;
@@ -512,14 +583,15 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
         size_t smem = (size_t)nbox * box_rows * W * sizeof(T);
         if (c->use_tma && (inner * sizeof(T)) % 16 == 0 && inner >= W && smem <= 200 * 1024 &&
             inner < (1L << 31) && outer < (1L << 31)) {
-            CUtensorMap tmap;
-            if (make_tensor_map_3d(&tmap, in, sizeof(T) == 8, (uint64_t)inner, (uint64_t)Nk, (uint64_t)outer,
-                                   (uint32_t)W, (uint32_t)box_rows)) {
-                static bool attr_set = false;
-                if (!attr_set) {
-                    cudaFuncSetAttribute(sweep_tile_tma_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-                    attr_set = true;
-                }
+            sldg_ctx::TmapSlot &ts = c->tmap3[dim][c->cur];
+            if (!ts.valid || ts.p0 != W || ts.p1 != box_rows) {
+                ts.valid = make_tensor_map_3d(&ts.map, in, sizeof(T) == 8, (uint64_t)inner, (uint64_t)Nk, (uint64_t)outer,
+                                              (uint32_t)W, (uint32_t)box_rows);
+                ts.p0 = W; ts.p1 = box_rows;
+            }
+            if (ts.valid) {
+                const CUtensorMap &tmap = ts.map;
+                CUDA_TRY(c, ensure_smem(c, sweep_tile_tma_kernel<T, O>, smem));
                 int nseg = 128 / W;
                 int cps = (int)cdiv(n, nseg);
                 long tpo = cdiv(inner, W);
@@ -603,14 +675,9 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
         const size_t slab_bytes = (size_t)O * n1 * O * sizeof(T);
         const size_t slot = (slab_bytes + 127) & ~(size_t)127;
         const long planes = midN * outer2;           // midN == 1 for (0, 1)
-        const char *e = getenv("SLDG_NO_PLANE_PAIR");
-        if (c->use_tma && !(e && e[0] == '1') && k1 == 0 && k2 == 1 && slab_bytes % 16 == 0 && 4 * slot <= 96 * 1024 &&
+        if (c->use_tma && c->tune.plane_pair && k1 == 0 && k2 == 1 && slab_bytes % 16 == 0 && 4 * slot <= 96 * 1024 &&
             n1 <= 256 && n2 >= 3 && planes < (1L << 31)) {
-            static bool attr_set = false;
-            if (!attr_set) {
-                cudaFuncSetAttribute(sweep_xpair_plane_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
-                attr_set = true;
-            }
+            CUDA_TRY(c, ensure_smem(c, sweep_xpair_plane_kernel<T, O>, 4 * slot));
             int blk = (int)(cdiv(n1, 32) * 32);
             sweep_xpair_plane_kernel<T, O><<<(unsigned)planes, blk, 4 * slot, c->stream>>>(
                 in, out, n1, n2, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2, (const T *)c->d_ab2, count2,
@@ -624,20 +691,21 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
     // v_a v_b at o >= 3: TMA-tile staged kernel for |shift| < 1 (lanes along inner1, per-cell tensor boxes);
     // at o <= 2 the register kernel below is as fast
     {
-        const char *e = getenv("SLDG_TILE_PAIR");        // 0 = never, 1 = also at o <= 2
-        const bool want = e ? (e[0] == '1') : (O >= 3);
+        // SLDG_TILE_PAIR: 0 = never, 1 = also at o <= 2
+        const bool want = c->tune.tile_pair >= 0 ? (c->tune.tile_pair == 1) : (O >= 3);
         const long blocks = (inner1 / 32) * (n1 / 4) * outer2;
-        if (c->use_tma && want && !(e && e[0] == '0') && k1 >= c->dx && midN == 1 && inner1 % 32 == 0 && n1 % 4 == 0 &&
+        if (c->use_tma && want && k1 >= c->dx && midN == 1 && inner1 % 32 == 0 && n1 % 4 == 0 &&
             n1 >= 4 && n2 >= 3 && inner1 < (1L << 31) && outer2 < (1L << 31) && blocks < (1L << 31)) {
-            CUtensorMap tmap;
-            if (make_tensor_map_4d(&tmap, in, sizeof(T) == 8, (uint64_t)inner1, (uint64_t)n1 * O, (uint64_t)n2 * O,
-                                   (uint64_t)outer2, 32, O, O)) {
+            sldg_ctx::TmapSlot &ts = c->tmap4[k1][c->cur];
+            if (!ts.valid || ts.p0 != k2) {
+                ts.valid = make_tensor_map_4d(&ts.map, in, sizeof(T) == 8, (uint64_t)inner1, (uint64_t)n1 * O,
+                                              (uint64_t)n2 * O, (uint64_t)outer2, 32, O, O);
+                ts.p0 = k2;
+            }
+            if (ts.valid) {
+                const CUtensorMap &tmap = ts.map;
                 const size_t smem = (size_t)3 * 6 * O * O * 32 * sizeof(T);
-                static bool attr_set = false;
-                if (!attr_set) {
-                    cudaFuncSetAttribute(sweep_vpair_tile_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-                    attr_set = true;
-                }
+                CUDA_TRY(c, ensure_smem(c, sweep_vpair_tile_kernel<T, O>, smem));
                 sweep_vpair_tile_kernel<T, O><<<(unsigned)blocks, 128, smem, c->stream>>>(
                     tmap, in, out, inner1, n1, n2, outer2, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2,
                     (const T *)c->d_ab2, count2, qd2, qm2);
@@ -712,11 +780,7 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
         const size_t slot = (slab_bytes + 127) & ~(size_t)127;
         if (c->use_tma && k1 == 0 && k2 == 1 && k3 == 2 && c->dx == 3 && slab_bytes % 16 == 0 &&
             4 * slot <= 200 * 1024 && (long)n1 * n2 <= 512 && outer3 < (1L << 31)) {
-            static bool attr_set = false;
-            if (!attr_set) {
-                cudaFuncSetAttribute(sweep_xtriple_plane_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-                attr_set = true;
-            }
+            CUDA_TRY(c, ensure_smem(c, sweep_xtriple_plane_kernel<T, O>, 4 * slot));
             int block = (int)(cdiv((long)n1 * n2, 32) * 32);
             sweep_xtriple_plane_kernel<T, O><<<(unsigned)outer3, block, 4 * slot, c->stream>>>(
                 in, out, n1, n2, n3, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2,
@@ -728,28 +792,42 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
         }
     }
     // v_a v_b v_c in the physical regime |shift| < 1: TMA-tile staged kernel
-    {
-        const char *e = getenv("SLDG_NO_TILE_TRIPLE");
-        const long blocks = (inner1 / 32) * (n1 / 4) * (n2 / 4) * outer3;
-        if (c->use_tma && !(e && e[0] == '1') && k1 >= c->dx && mid12 == 1 && mid23 == 1 && inner1 % 32 == 0 &&
-            n1 % 4 == 0 && n2 % 4 == 0 && n3 >= 3 && inner1 < (1L << 31) && blocks < (1L << 31)) {
-            CUtensorMap tmap;
-            if (make_tensor_map_5d(&tmap, in, sizeof(T) == 8, (uint64_t)inner1, (uint64_t)n1 * O, (uint64_t)n2 * O,
-                                   (uint64_t)n3 * O, (uint64_t)outer3, 32, O, O, O)) {
-                const size_t smem = (size_t)2 * 36 * O * O * O * 32 * sizeof(T);
-                static bool attr_set = false;
-                if (!attr_set) {
-                    cudaFuncSetAttribute(sweep_vtriple_tile_kernel<T, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-                    attr_set = true;
-                }
-                sweep_vtriple_tile_kernel<T, O><<<(unsigned)blocks, 512, smem, c->stream>>>(
-                    tmap, in, out, inner1, n1, n2, n3, outer3, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1],
-                    (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
-                LAUNCH_CHECK(c);
-                c->cur ^= 1;
-                c->have_rho = false;
-                return SLDG_OK;
+    if (c->use_tma && c->tune.tile_triple && k1 >= c->dx && mid12 == 1 && mid23 == 1 && n1 % 4 == 0 && n2 % 4 == 0 &&
+        n3 >= 3 && inner1 < (1L << 31)) {
+        // variants (columns W, ring depth NS, resident blocks): SLDG_VTRIPLE_VARIANT picks one for A/B runs
+        auto launch = [&](auto kern, int W, int NS) -> int {
+            const long blocks = (inner1 / W) * (n1 / 4) * (n2 / 4) * outer3;
+            if (inner1 % W || (W * sizeof(T)) % 16 || blocks >= (1L << 31)) return 1;          // not applicable
+            sldg_ctx::TmapSlot &ts = c->tmap5[c->cur];
+            if (!ts.valid || ts.p0 != W) {
+                ts.valid = make_tensor_map_5d(&ts.map, in, sizeof(T) == 8, (uint64_t)inner1, (uint64_t)n1 * O,
+                                              (uint64_t)n2 * O, (uint64_t)n3 * O, (uint64_t)outer3, W, O, O, O);
+                ts.p0 = W;
             }
+            if (!ts.valid) return 1;
+            const size_t smem = (size_t)NS * 36 * O * O * O * W * sizeof(T);
+            if (ensure_smem(c, kern, smem) != cudaSuccess) { cudaGetLastError(); return 1; }
+            kern<<<(unsigned)blocks, W * 16, smem, c->stream>>>(
+                ts.map, in, out, inner1, n1, n2, n3, outer3, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1],
+                (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+            return 0;
+        };
+        int rc = 1;
+        switch (c->tune.vt_variant) {
+        case 0: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 1>, 32, 2); break;
+        case 1: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 3, 2>, 16, 3); break;
+        case 2: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 4, 1>, 16, 4); break;
+        case 3: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 2, 3>, 16, 2); break;
+        case 4: rc = launch(sweep_vtriple_tile_kernel<T, O, 8, 3, 4>, 8, 3); break;
+        case 5: rc = launch(sweep_vtriple_tile_kernel<T, O, 8, 6, 2>, 8, 6); break;
+        case 6: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 3, 1>, 16, 3); break;
+        default: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 1>, 32, 2); break;
+        }
+        if (rc == 0) {
+            LAUNCH_CHECK(c);
+            c->cur ^= 1;
+            c->have_rho = false;
+            return SLDG_OK;
         }
     }
     int chunk = 32;
@@ -795,6 +873,7 @@ long sweep_count(const sldg_ctx *c, int dim) { return dim < c->dx ? c->N[c->dx +
 
 extern "C" int sldg_translate(sldg_ctx *c, int dim, const double *shift, size_t count) {
     if (!c || !shift || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     if ((long)count != sweep_count(c, dim))
         return fail(c, SLDG_ERR_ARG, "sldg_translate: dim %d needs %ld shifts, got %zu", dim, sweep_count(c, dim), count);
     use_tab(c, 1, c->gen[0], false);
@@ -805,6 +884,7 @@ extern "C" int sldg_translate(sldg_ctx *c, int dim, const double *shift, size_t 
 
 extern "C" int sldg_translate_dev(sldg_ctx *c, int dim, const double *shift, size_t count) {
     if (!c || !shift || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     if ((long)count != sweep_count(c, dim))
         return fail(c, SLDG_ERR_ARG, "sldg_translate_dev: dim %d needs %ld shifts, got %zu", dim, sweep_count(c, dim), count);
     use_tab(c, 1, c->gen[0], false);
@@ -823,11 +903,14 @@ int physics_tab(sldg_ctx *c, int slot, int dim, double dt) {
         if (t.valid && t.tau == dt) { use_tab(c, slot, t, true); return SLDG_OK; }
         use_tab(c, slot, t, false);
         int va = c->dx + dim;
+        // the table is being rewritten: not valid until the sweep that assembles it has been enqueued
+        // successfully (commit_tables); a failure in between leaves it invalid, never half-written-but-trusted
+        t.valid = false;
+        t.pending = true;
+        t.pending_tau = dt;
+        c->xt_epoch++;                  // graphs captured against the old table must not be replayed
         sigma_from_coords_kernel<<<(unsigned)cdiv(count, block), block, 0, c->stream>>>(
             c->d_coords[va], count, dt, c->h[dim], t.sigma);
-        t.tau = dt;
-        t.valid = true;                 // the assembly is enqueued by the sweep that follows
-        c->xt_epoch++;
     } else {
         int a = dim - c->dx;
         if (a >= c->dx) return fail(c, SLDG_ERR_ARG, "sldg_advect: v_%d has no field component (dx = %d)", a + 1, c->dx);
@@ -841,6 +924,16 @@ int physics_tab(sldg_ctx *c, int slot, int dim, double dt) {
     return SLDG_OK;
 }
 
+// after the sweep(s) that assemble the pending cached x-tables were enqueued: rc == 0 makes them valid
+int commit_tables(sldg_ctx *c, int rc) {
+    for (auto &t : c->xt)
+        if (t.pending) {
+            t.pending = false;
+            if (rc == SLDG_OK) { t.valid = true; t.tau = t.pending_tau; }
+        }
+    return rc;
+}
+
 bool pair_ok(const sldg_ctx *c, int d1, int d2) {
     if (d1 < 0 || d2 <= d1 || d2 >= c->D) return false;
     return (d2 < c->dx) || (d1 >= c->dx);          // both x-dimensions or both v-dimensions
@@ -849,9 +942,10 @@ bool pair_ok(const sldg_ctx *c, int d1, int d2) {
 
 extern "C" int sldg_advect(sldg_ctx *c, int dim, double dt) {
     if (!c || dim < 0 || dim >= c->D) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     int rc = physics_tab(c, 1, dim, dt);
-    if (rc) return rc;
-    return run_sweep(c, dim, sweep_count(c, dim));
+    if (rc) return commit_tables(c, rc);
+    return commit_tables(c, run_sweep(c, dim, sweep_count(c, dim)));
 }
 
 extern "C" int sldg_advect_pair(sldg_ctx *c, int dim1, int dim2, double dt) {
@@ -862,15 +956,17 @@ extern "C" int sldg_advect_pair(sldg_ctx *c, int dim1, int dim2, double dt) {
         int r1 = sldg_advect(c, dim1, dt);
         return r1 ? r1 : sldg_advect(c, dim2, dt);
     }
+    DeviceGuard guard(c);
     int rc = physics_tab(c, 1, dim1, dt);
-    if (rc) return rc;
-    if ((rc = physics_tab(c, 2, dim2, dt))) return rc;
-    return run_pair(c, dim1, dim2, sweep_count(c, dim1), sweep_count(c, dim2));
+    if (rc) return commit_tables(c, rc);
+    if ((rc = physics_tab(c, 2, dim2, dt))) return commit_tables(c, rc);
+    return commit_tables(c, run_pair(c, dim1, dim2, sweep_count(c, dim1), sweep_count(c, dim2)));
 }
 
 extern "C" int sldg_translate_pair_dev(sldg_ctx *c, int dim1, const double *shift1, size_t count1, int dim2,
                                        const double *shift2, size_t count2) {
     if (!c || !shift1 || !shift2) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     if (!pair_ok(c, dim1, dim2))
         return fail(c, SLDG_ERR_ARG, "sldg_translate_pair_dev: need dim1 < dim2, both x- or both v-dimensions");
     if ((long)count1 != sweep_count(c, dim1) || (long)count2 != sweep_count(c, dim2))
@@ -891,12 +987,12 @@ extern "C" int sldg_translate_pair_dev(sldg_ctx *c, int dim1, const double *shif
 // ------------------------------------------------------------------------------------------
 namespace {
 
-template <typename T, int VEC, bool S2, int UB>
+template <typename T, int VEC, bool S2, int UB, bool COMP = false>
 void launch_vsum(sldg_ctx *c, int splits, long vps, int block) {
     long xv = c->X / VEC;
     if (xv < block) block = (int)(cdiv(xv, 32) * 32);
     dim3 grid((unsigned)cdiv(xv, block), (unsigned)splits);
-    vsum_partial_kernel<T, VEC, S2, UB><<<grid, block, 0, c->stream>>>(
+    vsum_partial_kernel<T, VEC, S2, UB, COMP><<<grid, block, 0, c->stream>>>(
         (const T *)c->buf[c->cur], c->X, c->V, vps, c->d_Wv, c->d_part,
         c->d_part + (size_t)c->max_splits * c->X);
 }
@@ -909,15 +1005,16 @@ int run_vsum(sldg_ctx *c, double *rho_copy) {
     long s = cdiv(target, c->X / vec > 0 ? c->X / vec : 1);
     if (s > c->max_splits) s = c->max_splits;
     if (s < 1) s = 1;
-    // Small problems (the 1+1 D configs): one split, i.e. every x sums its v-nodes in ascending
-    // canonical order with fp64 multiply-then-add -- the order D:O4 states.  rho + 1 is a
-    // difference of O(1) sums (D:R11), so the summation order is visible at 1e-13 relative in E
-    // when the perturbation is 1e-3; large problems need the splits for parallelism.
+    // Small problems (the 1+1 D configs): one split, every x sums its v-nodes alone -- with a
+    // compensated accumulator, so that rho is the exactly summed value rounded once (D:O4).  rho + 1
+    // is a difference of O(1) sums (D:R11): a plain running sum is visible at 1e-13 relative in E
+    // when the perturbation is 1e-3.  Large problems need the splits for parallelism; their partials
+    // are short sums and the pass over the splits is compensated.
     const bool small = c->V * c->X <= (1L << 23);
     if (small) s = 1;
     long vps = cdiv(c->V, s);
     int splits = (int)cdiv(c->V, vps);
-    if (small) launch_vsum<T, 1, S2, 32>(c, splits, vps, 32);     // thread per x, 32 rows in flight
+    if (small) launch_vsum<T, 1, S2, 32, true>(c, splits, vps, 32);     // thread per x, 32 rows in flight
     else if (vec == VMAX) launch_vsum<T, VMAX, S2, 8>(c, splits, vps, 128);
     else if (vec == 2) launch_vsum<T, 2, S2, 8>(c, splits, vps, 128);
     else launch_vsum<T, 1, S2, 8>(c, splits, vps, 128);
@@ -1000,17 +1097,20 @@ int run_poisson(sldg_ctx *c, double *E_copy) {
 
 extern "C" int sldg_compute_rho(sldg_ctx *c, double *rho_out) {
     if (!c) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     return run_rho(c, rho_out, false);
 }
 
 extern "C" int sldg_poisson_E(sldg_ctx *c, double *E_out) {
     if (!c) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     if (!c->have_rho) return fail(c, SLDG_ERR_STATE, "sldg_poisson_E: rho of the current f not computed");
     return run_poisson(c, E_out);
 }
 
 extern "C" int sldg_set_E(sldg_ctx *c, const double *E, int is_device) {
     if (!c || !E) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     CUDA_TRY(c, cudaMemcpyAsync(c->d_E, E, (size_t)c->dx * c->X * sizeof(double),
                                 is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
     if (!is_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
@@ -1026,17 +1126,19 @@ extern "C" int sldg_advect_triple(sldg_ctx *c, int dim1, int dim2, int dim3, dou
         int r = sldg_advect_pair(c, dim1, dim2, dt);
         return r ? r : sldg_advect(c, dim3, dt);
     }
+    DeviceGuard guard(c);
     int rc;
-    if ((rc = physics_tab(c, 1, dim1, dt))) return rc;
-    if ((rc = physics_tab(c, 2, dim2, dt))) return rc;
-    if ((rc = physics_tab(c, 3, dim3, dt))) return rc;
-    return run_triple(c, dim1, dim2, dim3, sweep_count(c, dim1), sweep_count(c, dim2), sweep_count(c, dim3));
+    if ((rc = physics_tab(c, 1, dim1, dt))) return commit_tables(c, rc);
+    if ((rc = physics_tab(c, 2, dim2, dt))) return commit_tables(c, rc);
+    if ((rc = physics_tab(c, 3, dim3, dt))) return commit_tables(c, rc);
+    return commit_tables(c, run_triple(c, dim1, dim2, dim3, sweep_count(c, dim1), sweep_count(c, dim2), sweep_count(c, dim3)));
 }
 
 extern "C" int sldg_translate_triple_dev(sldg_ctx *c, int dim1, const double *shift1, size_t count1, int dim2,
                                          const double *shift2, size_t count2, int dim3, const double *shift3,
                                          size_t count3) {
     if (!c || !shift1 || !shift2 || !shift3) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     if (!pair_ok(c, dim1, dim2) || !pair_ok(c, dim2, dim3) || !pair_ok(c, dim1, dim3))
         return fail(c, SLDG_ERR_ARG, "sldg_translate_triple_dev: need dim1 < dim2 < dim3, all x- or all v-dimensions");
     if ((long)count1 != sweep_count(c, dim1) || (long)count2 != sweep_count(c, dim2) ||
@@ -1087,19 +1189,27 @@ int capture_step(sldg_ctx *c, double dt, sldg_ctx::StepGraph &g) {
         CUDA_TRY(c, cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking));
     if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
     cudaStream_t user = c->stream;
+    // nothing executes during a capture: on ANY failure the bookkeeping below is put back, so that the
+    // caller can run the step eagerly from exactly the state it had
     const int cur_in = c->cur;
     const unsigned long long l0 = c->launches;
+    const bool rho_in = c->have_rho, E_in = c->have_E;
+    auto restore = [&]() { c->cur = cur_in; c->launches = l0; c->have_rho = rho_in; c->have_E = E_in; };
     CUDA_TRY(c, cudaStreamBeginCapture(c->capture_stream, cudaStreamCaptureModeThreadLocal));
     c->stream = c->capture_stream;
     int rc = step_body(c, dt);
     c->stream = user;
     cudaGraph_t graph = nullptr;
     cudaError_t e = cudaStreamEndCapture(c->capture_stream, &graph);
-    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
-    if (e != cudaSuccess) return fail(c, SLDG_ERR_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+    if (rc) { if (graph) cudaGraphDestroy(graph); restore(); return rc; }
+    if (e != cudaSuccess) { restore(); return fail(c, SLDG_ERR_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e)); }
     e = cudaGraphInstantiate(&g.exec, graph, 0);
     cudaGraphDestroy(graph);
-    if (e != cudaSuccess) { g.exec = nullptr; return fail(c, SLDG_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e)); }
+    if (e != cudaSuccess) {
+        g.exec = nullptr;
+        restore();
+        return fail(c, SLDG_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+    }
     g.dt = dt; g.cur_in = cur_in; g.cur_out = c->cur; g.launches = c->launches - l0;
     g.xt_epoch = c->xt_epoch;
     return SLDG_OK;
@@ -1108,6 +1218,7 @@ int capture_step(sldg_ctx *c, double dt, sldg_ctx::StepGraph &g) {
 
 extern "C" int sldg_step(sldg_ctx *c, double dt) {
     if (!c) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     if (!c->use_graph) return step_body(c, dt);
     const int p = c->cur;
     sldg_ctx::StepGraph &g = c->graphs[p];
@@ -1120,9 +1231,14 @@ extern "C" int sldg_step(sldg_ctx *c, double dt) {
     if (c->eager_seen[p] && c->last_eager_dt[p] == dt && c->eager_epoch[p] == c->xt_epoch) {
         // second step with this (dt, parity) and untouched x-tables: capture (no table kernels inside)
         int rc = capture_step(c, dt, g);
-        if (rc) return rc;
-        CUDA_TRY(c, cudaGraphLaunch(g.exec, c->stream));
-        return SLDG_OK;
+        if (rc == SLDG_OK) {
+            CUDA_TRY(c, cudaGraphLaunch(g.exec, c->stream));
+            return SLDG_OK;
+        }
+        // capture or instantiation failed (state restored): graphs off for this context, step eagerly
+        cudaGetLastError();
+        c->use_graph = false;
+        return step_body(c, dt);
     }
     // first step with this (dt, parity): eager (it also fills the cached x-tables and kernel attributes)
     c->eager_seen[p] = true;
@@ -1167,6 +1283,7 @@ int run_moments(sldg_ctx *c) {
 
 extern "C" int sldg_moments(sldg_ctx *c, double *momentum, double *kinetic) {
     if (!c) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     int rc = c->dtype == SLDG_F64 ? run_moments<double>(c) : run_moments<float>(c);
     if (rc) return rc;
     double h[4];
@@ -1179,6 +1296,7 @@ extern "C" int sldg_moments(sldg_ctx *c, double *momentum, double *kinetic) {
 
 extern "C" int sldg_diagnostics(sldg_ctx *c, double *mass, double *l2, double *ee) {
     if (!c) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
     int rc;
     if ((rc = run_rho(c, nullptr, true))) return rc;
     if ((rc = run_poisson(c, nullptr))) return rc;

@@ -804,14 +804,19 @@ namespace sldg {
 // its O^3 window along k3, consumes stage j at local step j (m3 = n3-1) or j-1 (m3 = 0).
 // Bit-identical to the three sweeps; per-block fallback to direct global reads otherwise.
 // ------------------------------------------------------------------------------------------
-template <typename T, int O>
-__global__ void __launch_bounds__(512, 1)
+// W = columns (lanes along inner1) per block, NS = ring depth, MINB = blocks per SM the register
+// allocation is bounded for; block = W x 4 x 4 threads.  The kernel is bound by the latency of its
+// ring (ncu r2: 25 % of the warp samples wait for a stage to land, 14 % at the block barrier, DRAM
+// 58 %, L2 35 % with W = 32, NS = 2, one block of 512 threads per SM): narrower tiles make a stage
+// small enough for a deeper ring AND a second resident block.
+template <typename T, int O, int W, int NS, int MINB>
+__global__ void __launch_bounds__(W * 16, MINB)
 sweep_vtriple_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__restrict__ in, T *__restrict__ out,
                           long inner1, int n1, int n2, int n3, long outer3,
                           const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
                           const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2,
                           const int *__restrict__ mtab3, const T *__restrict__ ab3, long count3, long qdiv3, long qmod3) {
-    constexpr int W = 32, C1 = 4, C2 = 4, NS = 2;
+    constexpr int C1 = 4, C2 = 4;
     constexpr int CELL = O * O * O * W;                      // elements of one (k3, k2, k1)-cell box
     constexpr int STAGE = (C1 + 2) * (C2 + 2) * CELL;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
