@@ -138,8 +138,8 @@ int sldg_set_E(sldg_ctx *ctx, const double *E, int is_device);
 int sldg_step(sldg_ctx *ctx, double dt);
 
 /* mass = sum W f, l2 = sqrt(sum W f^2), electric_energy = 1/2 sum_x W_x |E|^2 from the
- * current f (D:R12); recomputes rho and E; synchronises the stream.  Any of the three
- * output pointers (host) may be NULL. */
+ * current f (D:R12); recomputes rho and E (they describe the current f afterwards); synchronises the
+ * stream.  Any of the three output pointers (host) may be NULL. */
 int sldg_diagnostics(sldg_ctx *ctx, double *mass, double *l2, double *electric_energy);
 
 /* S:8(f) NEXT-4 ("physical invariants", P:224 momentum conservation, Fig. 15 kinetic / total
@@ -147,6 +147,15 @@ int sldg_diagnostics(sldg_ctx *ctx, double *mass, double *l2, double *electric_e
  * kinetic_energy = 1/2 int int |v|^2 f dx dv from the current f; one read of f; synchronises the
  * stream.  Either pointer may be NULL.  Total energy = kinetic_energy + electric_energy. */
 int sldg_moments(sldg_ctx *ctx, double *momentum, double *kinetic_energy);
+
+/* All invariants the paper writes once per time step ("once at the beginning of the time step
+ * to write the electric energy and other invariant") in ONE read of the current f: the pass that forms
+ * rho also forms sum W f^2, sum v_a W f and sum |v|^2 W f (S:8(f) NEXT-4 "fused into the rho pass").
+ * Outputs as in sldg_diagnostics / sldg_moments (host pointers, any may be NULL; momentum has dv entries);
+ * synchronises the stream once.  The library remembers the result until f changes: sldg_diagnostics,
+ * sldg_moments and sldg_invariants called in any order on the same f read it from HBM once. */
+int sldg_invariants(sldg_ctx *ctx, double *mass, double *l2, double *electric_energy, double *momentum,
+                    double *kinetic_energy);
 
 /* Number of kernels this context has launched since sldg_create (bench "gpu_launches"). */
 unsigned long long sldg_launch_count(const sldg_ctx *ctx);

@@ -29,13 +29,12 @@ __device__ __forceinline__ void comp_add_product(double &hi, double &lo, double 
     two_sum_acc(hi, lo, p);
 }
 
-// part_rho[split][x] = sum_{v in split} W_v f[v][x];  part_s2 likewise with f^2 (if WITH_S2)
-// COMP: compensated accumulation of the rho sum (one-split launches: the partial IS rho).
-template <typename T, int VEC, bool WITH_S2, int UB, bool COMP = false>
+// part_rho[split][x] = sum_{v in split} W_v f[v][x]   (the rho pass of the Strang step: rho only)
+// COMP: compensated accumulation (one-split launches: the partial IS rho).
+template <typename T, int VEC, int UB, bool COMP = false>
 __global__ void __launch_bounds__(128)
 vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
-                    const double *__restrict__ Wv, double *__restrict__ part_rho,
-                    double *__restrict__ part_s2) {
+                    const double *__restrict__ Wv, double *__restrict__ part_rho) {
     using Vt = Vec<T, VEC>;
     const long xv = (long)blockIdx.x * blockDim.x + threadIdx.x;
     const long x = xv * VEC;
@@ -44,9 +43,9 @@ vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
     const long v0 = split * vps;
     long v1 = v0 + vps;
     if (v1 > V) v1 = V;
-    double acc[VEC], acc2[VEC], lo[VEC];
+    double acc[VEC], lo[VEC];
 #pragma unroll
-    for (int e = 0; e < VEC; ++e) { acc[e] = 0.0; acc2[e] = 0.0; lo[e] = 0.0; }
+    for (int e = 0; e < VEC; ++e) { acc[e] = 0.0; lo[e] = 0.0; }
     const T *p = f + v0 * X + x;
     long v = v0;
     for (; v + UB <= v1; v += UB) {
@@ -62,10 +61,8 @@ vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
 #pragma unroll
             for (int e = 0; e < VEC; ++e) {
                 double val = (double)u[b].v[e];
-                double wv = w[b] * val;
                 if (COMP) comp_add_product(acc[e], lo[e], w[b], val);
-                else acc[e] += wv;
-                if (WITH_S2) acc2[e] = fma(wv, val, acc2[e]);
+                else acc[e] += w[b] * val;
             }
         p += (long)UB * X;
     }
@@ -75,18 +72,13 @@ vsum_partial_kernel(const T *__restrict__ f, long X, long V, long vps,
 #pragma unroll
         for (int e = 0; e < VEC; ++e) {
             double val = (double)u.v[e];
-            double wv = w * val;
             if (COMP) comp_add_product(acc[e], lo[e], w, val);
-            else acc[e] += wv;
-            if (WITH_S2) acc2[e] = fma(wv, val, acc2[e]);
+            else acc[e] += w * val;
         }
         p += X;
     }
 #pragma unroll
-    for (int e = 0; e < VEC; ++e) {
-        part_rho[split * X + x + e] = COMP ? acc[e] + lo[e] : acc[e];
-        if (WITH_S2) part_s2[split * X + x + e] = acc2[e];
-    }
+    for (int e = 0; e < VEC; ++e) part_rho[split * X + x + e] = COMP ? acc[e] + lo[e] : acc[e];
 }
 
 __device__ __forceinline__ double warp_sum(double v);
@@ -158,50 +150,6 @@ scalars_kernel(const double *__restrict__ rho, const double *__restrict__ s2,
 
 namespace sldg {
 
-// S:8(f) NEXT-4 (Fig. 15): velocity moments per x-node,
-//   part[a][split][x] = sum_v v_a W_v f[v][x]  (a < DV),   part[DV][split][x] = sum_v |v|^2 W_v f[v][x],
-// one read of f, fp64 accumulators, same split structure as the rho pass.
-template <typename T, int VEC, int DV>
-__global__ void __launch_bounds__(128)
-vmoment_partial_kernel(const T *__restrict__ f, long X, long V, long vps, int nsplit_cap,
-                       const double *__restrict__ Wv, const double *__restrict__ va /* [DV][V] */,
-                       const double *__restrict__ v2, double *__restrict__ part) {
-    using Vt = Vec<T, VEC>;
-    const long xv = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long x = xv * VEC;
-    if (x >= X) return;
-    const long split = blockIdx.y;
-    const long v0 = split * vps;
-    long v1 = v0 + vps;
-    if (v1 > V) v1 = V;
-    double acc[DV + 1][VEC];
-#pragma unroll
-    for (int k = 0; k <= DV; ++k)
-#pragma unroll
-        for (int e = 0; e < VEC; ++e) acc[k][e] = 0.0;
-    const T *p = f + v0 * X + x;
-#pragma unroll 4
-    for (long v = v0; v < v1; ++v) {
-        Vt u = *reinterpret_cast<const Vt *>(p);
-        const double w = Wv[v], s2 = v2[v];
-        double c[DV];
-#pragma unroll
-        for (int a = 0; a < DV; ++a) c[a] = va[(long)a * V + v];
-#pragma unroll
-        for (int e = 0; e < VEC; ++e) {
-            const double wf = w * (double)u.v[e];
-#pragma unroll
-            for (int a = 0; a < DV; ++a) acc[a][e] += c[a] * wf;
-            acc[DV][e] += s2 * wf;
-        }
-        p += X;
-    }
-#pragma unroll
-    for (int k = 0; k <= DV; ++k)
-#pragma unroll
-        for (int e = 0; e < VEC; ++e) part[((long)k * nsplit_cap + split) * X + x + e] = acc[k][e];
-}
-
 // out[k] = sum_x W_x sum_split part[k][split][x], k < nk (one block of 1024 threads, fixed order)
 __global__ void __launch_bounds__(1024)
 moments_final_kernel(const double *__restrict__ part, const double *__restrict__ Wx, long X, int splits,
@@ -223,6 +171,79 @@ moments_final_kernel(const double *__restrict__ part, const double *__restrict__
             if (lane == 0) out[k] = a;
         }
         __syncthreads();
+    }
+}
+
+}  // namespace sldg
+
+namespace sldg {
+
+// S:8(f) NEXT-4 as the survey words it -- "fused into the rho pass" (P:69 lists the invariants together,
+// P:92 writes them once per step): ONE read of f emits, per x-node and v-split,
+//   part[0] = sum_v W_v f            (-> rho, mass)            part[1] = sum_v W_v f^2   (-> l2)
+//   part[2+a] = sum_v v_a W_v f      (-> momentum, a < DV)     part[2+DV] = sum_v |v|^2 W_v f (-> kinetic energy)
+// with fp64 accumulators and the split structure of the rho pass.  The rho and f^2 sums are the very
+// operations, in the very order, of vsum_partial_kernel<.., WITH_S2 = true, ..>, so sldg_diagnostics gives the
+// same bits whichever pass produced its partials.  COMP: compensated rho sum (one-split launches, D:O4).
+template <typename T, int VEC, int DV, int UB, bool COMP>
+__global__ void __launch_bounds__(128)
+vall_partial_kernel(const T *__restrict__ f, long X, long V, long vps, long part_stride /* cap * X */,
+                    const double *__restrict__ Wv, const double *__restrict__ va /* [DV][V] */,
+                    const double *__restrict__ v2, double *__restrict__ part) {
+    using Vt = Vec<T, VEC>;
+    const long xv = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long x = xv * VEC;
+    if (x >= X) return;
+    const long split = blockIdx.y;
+    const long v0 = split * vps;
+    long v1 = v0 + vps;
+    if (v1 > V) v1 = V;
+    double acc[VEC], lo[VEC], acc2[VEC], mom[DV + 1][VEC];
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) {
+        acc[e] = 0.0; lo[e] = 0.0; acc2[e] = 0.0;
+#pragma unroll
+        for (int k = 0; k <= DV; ++k) mom[k][e] = 0.0;
+    }
+    const T *p = f + v0 * X + x;
+    auto add_row = [&](const Vt &u, long v) {
+        const double w = Wv[v], s2 = v2[v];
+        double c[DV];
+#pragma unroll
+        for (int a = 0; a < DV; ++a) c[a] = va[(long)a * V + v];
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) {
+            const double val = (double)u.v[e];
+            const double wv = w * val;
+            if (COMP) comp_add_product(acc[e], lo[e], w, val);
+            else acc[e] += wv;
+            acc2[e] = fma(wv, val, acc2[e]);
+#pragma unroll
+            for (int a = 0; a < DV; ++a) mom[a][e] += c[a] * wv;
+            mom[DV][e] += s2 * wv;
+        }
+    };
+    long v = v0;
+    for (; v + UB <= v1; v += UB) {
+        Vt u[UB];
+#pragma unroll
+        for (int b = 0; b < UB; ++b) u[b] = *reinterpret_cast<const Vt *>(p + (long)b * X);
+#pragma unroll
+        for (int b = 0; b < UB; ++b) add_row(u[b], v + b);
+        p += (long)UB * X;
+    }
+    for (; v < v1; ++v) {
+        Vt u = *reinterpret_cast<const Vt *>(p);
+        add_row(u, v);
+        p += X;
+    }
+    double *o = part + split * X + x;
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) {
+        o[e] = COMP ? acc[e] + lo[e] : acc[e];
+        o[part_stride + e] = acc2[e];
+#pragma unroll
+        for (int k = 0; k <= DV; ++k) o[(2 + k) * part_stride + e] = mom[k][e];
     }
 }
 

@@ -82,8 +82,8 @@ struct sldg_ctx {
     double *d_va = nullptr, *d_v2 = nullptr;      // per v-node: coordinates v_a [dv][V] and |v|^2 [V]
     double *d_rho = nullptr, *d_s2 = nullptr, *d_E = nullptr;   // [X], [X], [dx][X]
     int max_splits = 1;
-    double *d_part = nullptr;          // [4][max_splits][X]
-    double *d_scal = nullptr;          // [8]
+    double *d_part = nullptr;          // [3 + dv][max_splits][X]: rho, f^2, v_a f, |v|^2 f partials
+    double *d_scal = nullptr;          // [8]: mass, l2^2, ee, momentum[dv], |v|^2 moment
     // Poisson
     long K[3] = {1, 1, 1}, Mmax[3] = {0, 0, 0}, KK = 1;
     double2 *d_F[3] = {nullptr, nullptr, nullptr}, *d_G[3] = {nullptr, nullptr, nullptr};
@@ -109,6 +109,7 @@ struct sldg_ctx {
     bool use_fuse = true;              // SLDG_NO_FUSE=1: sldg_step issues one sweep per pass
     bool use_tma = true;               // SLDG_NO_TMA=1 in the environment selects the plain kernels
     bool have_rho = false, have_E = false;
+    bool have_inv = false;             // d_part holds the one-read invariant partials of the CURRENT f
     unsigned long long launches = 0;
     char err[512] = "";
 };
@@ -142,6 +143,9 @@ int fail(sldg_ctx *c, int code, const char *fmt, ...) {
     } while (0)
 
 inline long cdiv(long a, long b) { return (a + b - 1) / b; }
+
+// f was (or is about to be) rewritten: everything derived from the old f is stale
+inline void f_changed(sldg_ctx *c) { c->have_rho = false; c->have_inv = false; }
 
 // Runs the enclosing entry point on the context's device, whatever device is current in the calling
 // thread, and restores the caller's device on return.
@@ -382,7 +386,7 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         if (s < 1) s = 1;
         if (s > 8192) s = 8192;
         c->max_splits = (int)s;
-        CREATE_TRY(dalloc(&c->d_part, (size_t)4 * c->max_splits * c->X));
+        CREATE_TRY(dalloc(&c->d_part, (size_t)(3 + dv) * c->max_splits * c->X));
     }
 
     // Poisson: dense DFT matrices per x-dimension (D:R6)
@@ -444,7 +448,7 @@ extern "C" int sldg_set_initial(sldg_ctx *c, const void *src, int is_device) {
     CUDA_TRY(c, cudaMemcpyAsync(c->buf[c->cur], src, bytes,
                                 is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
     if (!is_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    c->have_rho = false;
+    f_changed(c);
     return SLDG_OK;
 }
 
@@ -467,7 +471,7 @@ extern "C" int sldg_fill_uniform(sldg_ctx *c, unsigned long long seed, unsigned 
     else
         fill_uniform_kernel<float><<<blocks, 256, 0, c->stream>>>((float *)c->buf[c->cur], c->ndof, seed, tag);
     LAUNCH_CHECK(c);
-    c->have_rho = false;
+    f_changed(c);
     return SLDG_OK;
 }
 
@@ -604,7 +608,7 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
     }
     LAUNCH_CHECK(c);
     c->cur ^= 1;
-    c->have_rho = false;
+    f_changed(c);
     return SLDG_OK;
 }
 
@@ -684,7 +688,7 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
                 qd2, qm2);
             LAUNCH_CHECK(c);
             c->cur ^= 1;
-            c->have_rho = false;
+            f_changed(c);
             return SLDG_OK;
         }
     }
@@ -711,7 +715,7 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
                     (const T *)c->d_ab2, count2, qd2, qm2);
                 LAUNCH_CHECK(c);
                 c->cur ^= 1;
-                c->have_rho = false;
+                f_changed(c);
                 return SLDG_OK;
             }
         }
@@ -723,7 +727,7 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
             c->d_m2, (const T *)c->d_ab2, count2, qd2, qm2);
     LAUNCH_CHECK(c);
     c->cur ^= 1;
-    c->have_rho = false;
+    f_changed(c);
     return SLDG_OK;
 }
 
@@ -787,17 +791,18 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
                 qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
             LAUNCH_CHECK(c);
             c->cur ^= 1;
-            c->have_rho = false;
+            f_changed(c);
             return SLDG_OK;
         }
     }
     // v_a v_b v_c in the physical regime |shift| < 1: TMA-tile staged kernel
     if (c->use_tma && c->tune.tile_triple && k1 >= c->dx && mid12 == 1 && mid23 == 1 && n1 % 4 == 0 && n2 % 4 == 0 &&
-        n3 >= 3 && inner1 < (1L << 31)) {
-        // variants (columns W, ring depth NS, resident blocks): SLDG_VTRIPLE_VARIANT picks one for A/B runs
-        auto launch = [&](auto kern, int W, int NS) -> int {
-            const long blocks = (inner1 / W) * (n1 / 4) * (n2 / 4) * outer3;
-            if (inner1 % W || (W * sizeof(T)) % 16 || blocks >= (1L << 31)) return 1;          // not applicable
+        n3 >= 4 && inner1 < (1L << 31)) {
+        // variants (columns W, owned k2-cells C2, ring depth NS, resident blocks, drifting warps):
+        // SLDG_VTRIPLE_VARIANT picks one for A/B runs
+        auto launch = [&](auto kern, int W, int C2, int NS) -> int {
+            const long blocks = (inner1 / W) * (n1 / 4) * (n2 / C2) * outer3;
+            if (inner1 % W || n2 % C2 || (W * sizeof(T)) % 16 || blocks >= (1L << 31)) return 1;          // not applicable
             sldg_ctx::TmapSlot &ts = c->tmap5[c->cur];
             if (!ts.valid || ts.p0 != W) {
                 ts.valid = make_tensor_map_5d(&ts.map, in, sizeof(T) == 8, (uint64_t)inner1, (uint64_t)n1 * O,
@@ -805,28 +810,30 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
                 ts.p0 = W;
             }
             if (!ts.valid) return 1;
-            const size_t smem = (size_t)NS * 36 * O * O * O * W * sizeof(T);
+            const size_t smem = (size_t)NS * 6 * (C2 + 2) * O * O * O * W * sizeof(T);
             if (ensure_smem(c, kern, smem) != cudaSuccess) { cudaGetLastError(); return 1; }
-            kern<<<(unsigned)blocks, W * 16, smem, c->stream>>>(
+            kern<<<(unsigned)blocks, W * 4 * C2, smem, c->stream>>>(
                 ts.map, in, out, inner1, n1, n2, n3, outer3, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1],
                 (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
             return 0;
         };
         int rc = 1;
         switch (c->tune.vt_variant) {
-        case 0: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 1>, 32, 2); break;
-        case 1: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 3, 2>, 16, 3); break;
-        case 2: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 4, 1>, 16, 4); break;
-        case 3: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 2, 3>, 16, 2); break;
-        case 4: rc = launch(sweep_vtriple_tile_kernel<T, O, 8, 3, 4>, 8, 3); break;
-        case 5: rc = launch(sweep_vtriple_tile_kernel<T, O, 8, 6, 2>, 8, 6); break;
-        case 6: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 3, 1>, 16, 3); break;
-        default: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 1>, 32, 2); break;
+        case 0: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 4, 2, 1, false>, 32, 4, 2); break;
+        case 1: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 4, 3, 1, true>, 32, 4, 3); break;
+        case 2: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 2, 2, false>, 32, 2, 2); break;
+        case 3: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 3, 2, true>, 32, 2, 3); break;
+        case 4: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 4, 3, 2, false>, 16, 4, 3); break;
+        case 5: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 4, 4, 2, true>, 16, 4, 4); break;
+        case 6: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 4, 2, 1, true>, 32, 4, 2); break;
+        case 7: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 2, 2, false, false>, 32, 2, 2); break;
+        case 8: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 1, 2, 4, false>, 32, 1, 2); break;
+        default: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 2, 2, false>, 32, 2, 2); break;   // two resident blocks of 4 x 2 cells: 14.8 -> 13.9 ms at config 5
         }
         if (rc == 0) {
             LAUNCH_CHECK(c);
             c->cur ^= 1;
-            c->have_rho = false;
+            f_changed(c);
             return SLDG_OK;
         }
     }
@@ -845,7 +852,7 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
             mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
     LAUNCH_CHECK(c);
     c->cur ^= 1;
-    c->have_rho = false;
+    f_changed(c);
     return SLDG_OK;
 }
 
@@ -987,22 +994,17 @@ extern "C" int sldg_translate_pair_dev(sldg_ctx *c, int dim1, const double *shif
 // ------------------------------------------------------------------------------------------
 namespace {
 
-template <typename T, int VEC, bool S2, int UB, bool COMP = false>
-void launch_vsum(sldg_ctx *c, int splits, long vps, int block) {
-    long xv = c->X / VEC;
-    if (xv < block) block = (int)(cdiv(xv, 32) * 32);
-    dim3 grid((unsigned)cdiv(xv, block), (unsigned)splits);
-    vsum_partial_kernel<T, VEC, S2, UB, COMP><<<grid, block, 0, c->stream>>>(
-        (const T *)c->buf[c->cur], c->X, c->V, vps, c->d_Wv, c->d_part,
-        c->d_part + (size_t)c->max_splits * c->X);
-}
+int run_poisson_fwd(sldg_ctx *c);
 
-template <typename T, bool S2>
-int run_vsum(sldg_ctx *c, double *rho_copy) {
+// v-split geometry shared by the rho pass and the one-read invariants pass
+struct VSplit { int vec; long vps; int splits; bool small; };
+template <typename T>
+VSplit vsplit(const sldg_ctx *c) {
     constexpr int VMAX = 16 / (int)sizeof(T);
-    int vec = (c->X % VMAX == 0) ? VMAX : ((c->X % 2 == 0) ? 2 : 1);
+    VSplit g;
+    g.vec = (c->X % VMAX == 0) ? VMAX : ((c->X % 2 == 0) ? 2 : 1);
     long target = (long)c->sm_count * 2048 * 2;
-    long s = cdiv(target, c->X / vec > 0 ? c->X / vec : 1);
+    long s = cdiv(target, c->X / g.vec > 0 ? c->X / g.vec : 1);
     if (s > c->max_splits) s = c->max_splits;
     if (s < 1) s = 1;
     // Small problems (the 1+1 D configs): one split, every x sums its v-nodes alone -- with a
@@ -1010,28 +1012,98 @@ int run_vsum(sldg_ctx *c, double *rho_copy) {
     // is a difference of O(1) sums (D:R11): a plain running sum is visible at 1e-13 relative in E
     // when the perturbation is 1e-3.  Large problems need the splits for parallelism; their partials
     // are short sums and the pass over the splits is compensated.
-    const bool small = c->V * c->X <= (1L << 23);
-    if (small) s = 1;
-    long vps = cdiv(c->V, s);
-    int splits = (int)cdiv(c->V, vps);
-    if (small) launch_vsum<T, 1, S2, 32, true>(c, splits, vps, 32);     // thread per x, 32 rows in flight
-    else if (vec == VMAX) launch_vsum<T, VMAX, S2, 8>(c, splits, vps, 128);
-    else if (vec == 2) launch_vsum<T, 2, S2, 8>(c, splits, vps, 128);
-    else launch_vsum<T, 1, S2, 8>(c, splits, vps, 128);
-    LAUNCH_CHECK(c);
+    g.small = c->V * c->X <= (1L << 23);
+    if (g.small) { s = 1; g.vec = 1; }
+    g.vps = cdiv(c->V, s);
+    g.splits = (int)cdiv(c->V, g.vps);
+    return g;
+}
+
+template <typename T, int VEC, int UB, bool COMP = false>
+void launch_vsum(sldg_ctx *c, int splits, long vps, int block) {
+    long xv = c->X / VEC;
+    if (xv < block) block = (int)(cdiv(xv, 32) * 32);
+    dim3 grid((unsigned)cdiv(xv, block), (unsigned)splits);
+    vsum_partial_kernel<T, VEC, UB, COMP><<<grid, block, 0, c->stream>>>(
+        (const T *)c->buf[c->cur], c->X, c->V, vps, c->d_Wv, c->d_part);
+}
+
+// pass over the splits: rho (and s2 when the partials come from the invariants pass)
+int finish_vsum(sldg_ctx *c, int splits, double *rho_copy, bool with_s2) {
     int block = 256;
     vsum_final_kernel<<<(unsigned)cdiv(c->X * 32, block), block, 0, c->stream>>>(
-        c->d_part, S2 ? c->d_part + (size_t)c->max_splits * c->X : nullptr, c->X, splits, c->d_rho,
-        rho_copy, S2 ? c->d_s2 : nullptr);
+        c->d_part, with_s2 ? c->d_part + (size_t)c->max_splits * c->X : nullptr, c->X, splits, c->d_rho,
+        rho_copy, with_s2 ? c->d_s2 : nullptr);
     LAUNCH_CHECK(c);
     c->have_rho = true;
     return SLDG_OK;
 }
 
-int run_rho(sldg_ctx *c, double *rho_copy, bool with_s2) {
-    if (c->dtype == SLDG_F64)
-        return with_s2 ? run_vsum<double, true>(c, rho_copy) : run_vsum<double, false>(c, rho_copy);
-    return with_s2 ? run_vsum<float, true>(c, rho_copy) : run_vsum<float, false>(c, rho_copy);
+// a-3: rho only (the Strang step)
+template <typename T>
+int run_vsum(sldg_ctx *c, double *rho_copy) {
+    constexpr int VMAX = 16 / (int)sizeof(T);
+    const VSplit g = vsplit<T>(c);
+    c->have_inv = false;                                   // d_part is overwritten
+    if (g.small) launch_vsum<T, 1, 32, true>(c, g.splits, g.vps, 32);     // thread per x, 32 rows in flight
+    else if (g.vec == VMAX) launch_vsum<T, VMAX, 8>(c, g.splits, g.vps, 128);
+    else if (g.vec == 2) launch_vsum<T, 2, 8>(c, g.splits, g.vps, 128);
+    else launch_vsum<T, 1, 8>(c, g.splits, g.vps, 128);
+    LAUNCH_CHECK(c);
+    return finish_vsum(c, g.splits, rho_copy, false);
+}
+
+int run_rho(sldg_ctx *c, double *rho_copy) {
+    return c->dtype == SLDG_F64 ? run_vsum<double>(c, rho_copy) : run_vsum<float>(c, rho_copy);
+}
+
+// a-6 + NEXT-4: ONE read of the current f leaves the partials of rho, f^2, v_a f and |v|^2 f in d_part
+// (vall_partial_kernel) and rho, s2 in d_rho, d_s2; remembered until f changes, so that
+// sldg_diagnostics followed by sldg_moments (or sldg_invariants) reads f once.
+template <typename T, int VEC, int DV, int UB, bool COMP>
+void launch_vall(sldg_ctx *c, int splits, long vps, int block) {
+    long xv = c->X / VEC;
+    if (xv < block) block = (int)(cdiv(xv, 32) * 32);
+    dim3 grid((unsigned)cdiv(xv, block), (unsigned)splits);
+    vall_partial_kernel<T, VEC, DV, UB, COMP><<<grid, block, 0, c->stream>>>(
+        (const T *)c->buf[c->cur], c->X, c->V, vps, (long)c->max_splits * c->X, c->d_Wv, c->d_va, c->d_v2,
+        c->d_part);
+}
+template <typename T, int DV>
+int run_vall_dv(sldg_ctx *c) {
+    constexpr int VMAX = 16 / (int)sizeof(T);
+    const VSplit g = vsplit<T>(c);
+    if (g.small) launch_vall<T, 1, DV, 16, true>(c, g.splits, g.vps, 32);
+    else if (g.vec == VMAX) launch_vall<T, VMAX, DV, 4, false>(c, g.splits, g.vps, 128);
+    else if (g.vec == 2) launch_vall<T, 2, DV, 8, false>(c, g.splits, g.vps, 128);
+    else launch_vall<T, 1, DV, 8, false>(c, g.splits, g.vps, 128);
+    LAUNCH_CHECK(c);
+    int rc = finish_vsum(c, g.splits, nullptr, true);
+    if (rc) return rc;
+    // momentum and |v|^2 moment: sum over splits and x of partials 2 .. 2+dv -> d_scal[3 .. 3+dv]
+    moments_final_kernel<<<1, 1024, 0, c->stream>>>(c->d_part + (size_t)2 * c->max_splits * c->X, c->d_Wx, c->X,
+                                                    g.splits, c->max_splits, c->dv + 1, c->d_scal + 3);
+    LAUNCH_CHECK(c);
+    c->have_inv = true;
+    return SLDG_OK;
+}
+template <typename T>
+int run_vall_t(sldg_ctx *c) {
+    if (c->dv == 1) return run_vall_dv<T, 1>(c);
+    if (c->dv == 2) return run_vall_dv<T, 2>(c);
+    return run_vall_dv<T, 3>(c);
+}
+// all invariants of the current f into d_scal[0 .. 3+dv] (no read of f when they are already there)
+int run_invariants(sldg_ctx *c) {
+    int rc;
+    if (!c->have_inv) {
+        rc = c->dtype == SLDG_F64 ? run_vall_t<double>(c) : run_vall_t<float>(c);
+        if (rc) return rc;
+        if ((rc = run_poisson_fwd(c))) return rc;
+        scalars_kernel<<<1, 1024, 0, c->stream>>>(c->d_rho, c->d_s2, c->d_E, c->d_Wx, c->X, c->dx, c->d_scal);
+        LAUNCH_CHECK(c);
+    }
+    return SLDG_OK;
 }
 
 // apply M (rows x cols) along dimension b of a complex tensor with extents shape[] (index 0 fastest)
@@ -1093,12 +1165,14 @@ int run_poisson(sldg_ctx *c, double *E_copy) {
     return SLDG_OK;
 }
 
+int run_poisson_fwd(sldg_ctx *c) { return run_poisson(c, nullptr); }
+
 }  // namespace
 
 extern "C" int sldg_compute_rho(sldg_ctx *c, double *rho_out) {
     if (!c) return SLDG_ERR_ARG;
     DeviceGuard guard(c);
-    return run_rho(c, rho_out, false);
+    return run_rho(c, rho_out);
 }
 
 extern "C" int sldg_poisson_E(sldg_ctx *c, double *E_out) {
@@ -1175,7 +1249,7 @@ namespace {
 int step_body(sldg_ctx *c, double dt) {
     int rc;
     if ((rc = advect_group(c, 0, c->dx, 0.5 * dt))) return rc;
-    if ((rc = run_rho(c, nullptr, false))) return rc;
+    if ((rc = run_rho(c, nullptr))) return rc;
     if ((rc = run_poisson(c, nullptr))) return rc;
     if ((rc = advect_group(c, c->dx, c->dx, dt))) return rc;
     if ((rc = advect_group(c, 0, c->dx, 0.5 * dt))) return rc;
@@ -1194,7 +1268,8 @@ int capture_step(sldg_ctx *c, double dt, sldg_ctx::StepGraph &g) {
     const int cur_in = c->cur;
     const unsigned long long l0 = c->launches;
     const bool rho_in = c->have_rho, E_in = c->have_E;
-    auto restore = [&]() { c->cur = cur_in; c->launches = l0; c->have_rho = rho_in; c->have_E = E_in; };
+    const bool inv_in = c->have_inv;
+    auto restore = [&]() { c->cur = cur_in; c->launches = l0; c->have_rho = rho_in; c->have_E = E_in; c->have_inv = inv_in; };
     CUDA_TRY(c, cudaStreamBeginCapture(c->capture_stream, cudaStreamCaptureModeThreadLocal));
     c->stream = c->capture_stream;
     int rc = step_body(c, dt);
@@ -1225,7 +1300,7 @@ extern "C" int sldg_step(sldg_ctx *c, double dt) {
     if (g.exec && g.dt == dt && g.cur_in == p && g.xt_epoch == c->xt_epoch) {   // replay
         CUDA_TRY(c, cudaGraphLaunch(g.exec, c->stream));
         c->cur = g.cur_out; c->launches += g.launches;
-        c->have_rho = false; c->have_E = true;
+        f_changed(c); c->have_E = true;
         return SLDG_OK;
     }
     if (c->eager_seen[p] && c->last_eager_dt[p] == dt && c->eager_epoch[p] == c->xt_epoch) {
@@ -1248,43 +1323,10 @@ extern "C" int sldg_step(sldg_ctx *c, double dt) {
     return rc;
 }
 
-namespace {
-template <typename T, int VEC, int DV>
-void launch_vmoment(sldg_ctx *c, int splits, long vps) {
-    int block = 128;
-    long xv = c->X / VEC;
-    if (xv < block) block = (int)(cdiv(xv, 32) * 32);
-    dim3 grid((unsigned)cdiv(xv, block), (unsigned)splits);
-    vmoment_partial_kernel<T, VEC, DV><<<grid, block, 0, c->stream>>>(
-        (const T *)c->buf[c->cur], c->X, c->V, vps, c->max_splits, c->d_Wv, c->d_va, c->d_v2, c->d_part);
-}
-template <typename T>
-int run_moments(sldg_ctx *c) {
-    constexpr int VMAX = 16 / (int)sizeof(T);
-    const int vec = (c->X % VMAX == 0) ? VMAX : 1;
-    long target = (long)c->sm_count * 2048 * 2;
-    long s = cdiv(target, c->X / vec > 0 ? c->X / vec : 1);
-    if (s > c->max_splits) s = c->max_splits;
-    if (s < 1) s = 1;
-    long vps = cdiv(c->V, s);
-    int splits = (int)cdiv(c->V, vps);
-#define MOM_CASE(DV)                                                   \
-    if (vec == VMAX) launch_vmoment<T, VMAX, DV>(c, splits, vps);      \
-    else launch_vmoment<T, 1, DV>(c, splits, vps);
-    if (c->dv == 1) { MOM_CASE(1) } else if (c->dv == 2) { MOM_CASE(2) } else { MOM_CASE(3) }
-#undef MOM_CASE
-    LAUNCH_CHECK(c);
-    moments_final_kernel<<<1, 1024, 0, c->stream>>>(c->d_part, c->d_Wx, c->X, splits, c->max_splits, c->dv + 1,
-                                                    c->d_scal + 3);
-    LAUNCH_CHECK(c);
-    return SLDG_OK;
-}
-}  // namespace
-
 extern "C" int sldg_moments(sldg_ctx *c, double *momentum, double *kinetic) {
     if (!c) return SLDG_ERR_ARG;
     DeviceGuard guard(c);
-    int rc = c->dtype == SLDG_F64 ? run_moments<double>(c) : run_moments<float>(c);
+    int rc = run_invariants(c);
     if (rc) return rc;
     double h[4];
     CUDA_TRY(c, cudaMemcpyAsync(h, c->d_scal + 3, (c->dv + 1) * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -1297,16 +1339,30 @@ extern "C" int sldg_moments(sldg_ctx *c, double *momentum, double *kinetic) {
 extern "C" int sldg_diagnostics(sldg_ctx *c, double *mass, double *l2, double *ee) {
     if (!c) return SLDG_ERR_ARG;
     DeviceGuard guard(c);
-    int rc;
-    if ((rc = run_rho(c, nullptr, true))) return rc;
-    if ((rc = run_poisson(c, nullptr))) return rc;
-    scalars_kernel<<<1, 1024, 0, c->stream>>>(c->d_rho, c->d_s2, c->d_E, c->d_Wx, c->X, c->dx, c->d_scal);
-    LAUNCH_CHECK(c);
+    int rc = run_invariants(c);
+    if (rc) return rc;
     double h[3];
     CUDA_TRY(c, cudaMemcpyAsync(h, c->d_scal, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     if (mass) *mass = h[0];
     if (l2) *l2 = sqrt(h[1]);
     if (ee) *ee = h[2];
+    return SLDG_OK;
+}
+
+extern "C" int sldg_invariants(sldg_ctx *c, double *mass, double *l2, double *ee, double *momentum,
+                               double *kinetic) {
+    if (!c) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
+    int rc = run_invariants(c);
+    if (rc) return rc;
+    double h[8];
+    CUDA_TRY(c, cudaMemcpyAsync(h, c->d_scal, (4 + c->dv) * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    if (mass) *mass = h[0];
+    if (l2) *l2 = sqrt(h[1]);
+    if (ee) *ee = h[2];
+    if (momentum) for (int a = 0; a < c->dv; ++a) momentum[a] = h[3 + a];
+    if (kinetic) *kinetic = 0.5 * h[3 + c->dv];
     return SLDG_OK;
 }

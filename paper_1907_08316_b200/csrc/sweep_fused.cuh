@@ -804,23 +804,27 @@ namespace sldg {
 // its O^3 window along k3, consumes stage j at local step j (m3 = n3-1) or j-1 (m3 = 0).
 // Bit-identical to the three sweeps; per-block fallback to direct global reads otherwise.
 // ------------------------------------------------------------------------------------------
-// W = columns (lanes along inner1) per block, NS = ring depth, MINB = blocks per SM the register
-// allocation is bounded for; block = W x 4 x 4 threads.  The kernel is bound by the latency of its
-// ring (ncu r2: 25 % of the warp samples wait for a stage to land, 14 % at the block barrier, DRAM
-// 58 %, L2 35 % with W = 32, NS = 2, one block of 512 threads per SM): narrower tiles make a stage
-// small enough for a deeper ring AND a second resident block.
-template <typename T, int O, int W, int NS, int MINB>
-__global__ void __launch_bounds__(W * 16, MINB)
+// W = columns (lanes along inner1) per block, C2 = owned k2-cells (C1 = 4 k1-cells), NS = ring depth, MINB =
+// blocks per SM the register allocation is bounded for; block = W x 4 x C2 threads.
+// ncu (profiles/ncu_vtile_r2.md): no unit is saturated (issue 33 %, fp64 26 %, LSU 26 %, L2 35 %, DRAM 58 %);
+// 20 % of the warp samples wait for a stage to land and 15 % at the block barrier that recycles a slot: every
+// warp of the single resident block is in the same phase at the same time.  DRIFT replaces that barrier by
+// per-slot "empty" mbarriers counted in warps: a warp releases a slot as soon as it has read its raw values and
+// goes on; only warp 0 (which issues the copies) waits for the others, one iteration later, before it refills.
+template <typename T, int O, int W, int C2, int NS, int MINB, bool DRIFT, bool EVF = true>
+__global__ void __launch_bounds__(W * 4 * C2, MINB)
 sweep_vtriple_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__restrict__ in, T *__restrict__ out,
                           long inner1, int n1, int n2, int n3, long outer3,
                           const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
                           const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2,
                           const int *__restrict__ mtab3, const T *__restrict__ ab3, long count3, long qdiv3, long qmod3) {
-    constexpr int C1 = 4, C2 = 4;
+    constexpr int C1 = 4;
+    constexpr int NBOX = (C1 + 2) * (C2 + 2);
+    constexpr int NWARP = W * C1 * C2 / 32;
     constexpr int CELL = O * O * O * W;                      // elements of one (k3, k2, k1)-cell box
-    constexpr int STAGE = (C1 + 2) * (C2 + 2) * CELL;
+    constexpr int STAGE = NBOX * CELL;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t full[NS];
+    __shared__ __align__(8) uint64_t full[NS], empty[NS];
     T *ring = reinterpret_cast<T *>(smem_raw);
 
     const long tiles_x = inner1 / W;
@@ -831,6 +835,7 @@ sweep_vtriple_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__r
     const long tx = b % tiles_x;
     const long oo3 = b / tiles_x;
     const int tid = threadIdx.x, col = tid % W, t1 = (tid / W) % C1, t2 = tid / (W * C1);
+    const int warp = tid >> 5, lane = tid & 31;
     const int c1 = g1 * C1 + t1, c2 = g2 * C2 + t2;
     const long ii = tx * W + col;
     const long s1 = inner1, s2 = (long)n1 * O * s1, s3 = (long)n2 * O * s2;
@@ -848,7 +853,7 @@ sweep_vtriple_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__r
     const int m1 = mtab1[q1], m2 = mtab2[q2], m3 = mtab3[q3];
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NWARP); }
     }
     const bool small = __syncthreads_and((m1 == 0 || m1 == n1 - 1) && (m2 == 0 || m2 == n2 - 1) &&
                                          (m3 == 0 || m3 == n3 - 1)) != 0;
@@ -859,28 +864,31 @@ sweep_vtriple_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__r
     const int la = t1 + (m1 == 0 ? 1 : 0), lb = t2 + (m2 == 0 ? 1 : 0);   // staged path: local source cells
     const int late = (m3 == 0) ? 1 : 0;
     // which neighbour columns / rows of cells the block really needs (a tile without a sign change of
-    // the field needs only one side: 25 instead of 36 cell pairs per 16 owned)
+    // the field needs only one side)
     const bool needL1 = __syncthreads_or(m1 != 0) != 0, needR1 = __syncthreads_or(m1 == 0) != 0;
     const bool needL2 = __syncthreads_or(m2 != 0) != 0, needR2 = __syncthreads_or(m2 == 0) != 0;
     const int nboxes = (C1 + (needL1 ? 1 : 0) + (needR1 ? 1 : 0)) * (C2 + (needL2 ? 1 : 0) + (needR2 ? 1 : 0));
 
-    auto issue = [&](int j) {                                // stage j <-> k3-cell (j - 1) mod n3; all threads call
+    auto issue = [&](int j) {                                // stage j <-> k3-cell (j - 1) mod n3; warp 0 calls
         int cell3 = j - 1;
         if (cell3 < 0) cell3 += n3;
         if (cell3 >= n3) cell3 -= n3;
         const int slot = j % NS;
-        if (tid == 0) mbar_expect_tx(&full[slot], (uint32_t)(nboxes * CELL * sizeof(T)));
-        const int ca = tid % (C1 + 2), cb = tid / (C1 + 2);
-        if (tid < (C1 + 2) * (C2 + 2) && (ca > 0 || needL1) && (ca < C1 + 1 || needR1) && (cb > 0 || needL2) &&
-            (cb < C2 + 1 || needR2)) {
-            int cell1 = g1 * C1 - 1 + ca;
-            if (cell1 < 0) cell1 += n1;
-            if (cell1 >= n1) cell1 -= n1;
-            int cell2 = g2 * C2 - 1 + cb;
-            if (cell2 < 0) cell2 += n2;
-            if (cell2 >= n2) cell2 -= n2;
-            tma_load_5d_hint(ring + (size_t)slot * STAGE + (size_t)tid * CELL, &tmap, (int)(tx * W), cell1 * O, cell2 * O,
-                             cell3 * O, (int)oo3, &full[slot], policy_evict_first());
+        if (lane == 0) mbar_expect_tx(&full[slot], (uint32_t)(nboxes * CELL * sizeof(T)));
+        const uint64_t pol = EVF ? policy_evict_first() : policy_evict_last();
+#pragma unroll
+        for (int bx = lane; bx < NBOX; bx += 32) {
+            const int ca = bx % (C1 + 2), cb = bx / (C1 + 2);
+            if ((ca > 0 || needL1) && (ca < C1 + 1 || needR1) && (cb > 0 || needL2) && (cb < C2 + 1 || needR2)) {
+                int cell1 = g1 * C1 - 1 + ca;
+                if (cell1 < 0) cell1 += n1;
+                if (cell1 >= n1) cell1 -= n1;
+                int cell2 = g2 * C2 - 1 + cb;
+                if (cell2 < 0) cell2 += n2;
+                if (cell2 >= n2) cell2 -= n2;
+                tma_load_5d_hint(ring + (size_t)slot * STAGE + (size_t)bx * CELL, &tmap, (int)(tx * W), cell1 * O,
+                                 cell2 * O, cell3 * O, (int)oo3, &full[slot], pol);
+            }
         }
     };
     auto k12_staged = [&](int slot, T (&w)[O][O][O]) {
@@ -937,7 +945,23 @@ sweep_vtriple_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__r
                 }
         }
     };
-    auto emit = [&](int i3, const T (&w0)[O][O][O], const T (&w1)[O][O][O]) {
+    // The k3 rule in two halves (same operations in the same order as chain<>: one multiply and O-1 FMAs with
+    // the A3 row on the older cell, then O FMAs with the B3 row on the newer one).  The A-half is taken as soon
+    // as a cell's (k1,k2)-swept values exist and replaces them as the thread's state, so no window is copied.
+    auto a_half = [&](const T (&w)[O][O][O], T (&acc)[O][O][O]) {
+#pragma unroll
+        for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a = mul_t<T>(A3[j3 * O], w[0][j2][j1]);
+#pragma unroll
+                    for (int l = 1; l < O; ++l) a = fma_t<T>(A3[j3 * O + l], w[l][j2][j1], a);
+                    acc[j3][j2][j1] = a;
+                }
+    };
+    auto b_half_store = [&](int i3, const T (&acc)[O][O][O], const T (&w)[O][O][O]) {
         T *dst = out + lin0 + (long)i3 * O * s3;
 #pragma unroll
         for (int j3 = 0; j3 < O; ++j3)
@@ -945,42 +969,51 @@ sweep_vtriple_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__r
             for (int j2 = 0; j2 < O; ++j2)
 #pragma unroll
                 for (int j1 = 0; j1 < O; ++j1) {
-                    T a0[O], a1[O];
+                    T a = acc[j3][j2][j1];
 #pragma unroll
-                    for (int l = 0; l < O; ++l) { a0[l] = w0[l][j2][j1]; a1[l] = w1[l][j2][j1]; }
-                    __stcs(dst + (long)j3 * s3 + (long)j2 * s2 + (long)j1 * s1, chain<T, O>(A3, B3, j3, a0, a1));
+                    for (int l = 0; l < O; ++l) a = fma_t<T>(B3[j3 * O + l], w[l][j2][j1], a);
+                    __stcs(dst + (long)j3 * s3 + (long)j2 * s2 + (long)j1 * s1, a);
                 }
     };
-    auto copy = [&](T (&d)[O][O][O], const T (&s)[O][O][O]) {
-#pragma unroll
-        for (int a = 0; a < O; ++a)
-#pragma unroll
-            for (int c = 0; c < O; ++c)
-#pragma unroll
-                for (int e = 0; e < O; ++e) d[a][c][e] = s[a][c][e];
-    };
 
-    T wfirst[O][O][O], w0[O][O][O], w1[O][O][O];
+    T wfirst[O][O][O], acc[O][O][O], w1[O][O][O];
     if (small) {
-        for (int j = 0; j < NS && j <= n3; ++j) issue(j);
+        if (warp == 0)
+            for (int j = 0; j < NS && j <= n3; ++j) issue(j);
         for (int j = 0; j <= n3 + 1; ++j) {
             const int t = j - late;
+            bool pending = false;
             if (j <= n3) {
+                if constexpr (DRIFT) {
+                    // refill the slot of stage j-1 (released by every warp during the previous iteration)
+                    if (warp == 0 && j >= 1 && j - 1 + NS <= n3) {
+                        mbar_wait(&empty[(j - 1) % NS], (uint32_t)(((j - 1) / NS) & 1));
+                        issue(j - 1 + NS);
+                    }
+                }
                 mbar_wait(&full[j % NS], (uint32_t)((j / NS) & 1));
                 if (t == 0) {
                     k12_staged(j % NS, wfirst);
-                    copy(w0, wfirst);
                 } else if (t >= 1 && t <= n3 - 1) {
                     k12_staged(j % NS, w1);
-                    emit(t - 1, w0, w1);
-                    copy(w0, w1);
+                    pending = true;
+                }
+                // the slot is free as soon as its raw values have been read: released BEFORE the k3 rule and
+                // the stores, so that the copy engine works during them
+                if constexpr (DRIFT) {
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&empty[j % NS]);
+                } else {
+                    __syncthreads();
+                    if (warp == 0 && j + NS <= n3) issue(j + NS);
                 }
             }
-            if (t == n3) emit(n3 - 1, w0, wfirst);
-            if (j <= n3) {
-                __syncthreads();
-                if (j + NS <= n3) issue(j + NS);
+            if (t == 0) a_half(wfirst, acc);
+            if (pending) {
+                b_half_store(t - 1, acc, w1);
+                a_half(w1, acc);
             }
+            if (t == n3) b_half_store(n3 - 1, acc, wfirst);  // closes the periodic line
         }
     } else {
         for (int t = 0; t <= n3; ++t) {
@@ -988,13 +1021,13 @@ sweep_vtriple_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__r
             if (cell3 >= n3) cell3 -= n3;
             if (t == 0) {
                 k12_global(cell3, wfirst);
-                copy(w0, wfirst);
+                a_half(wfirst, acc);
             } else if (t <= n3 - 1) {
                 k12_global(cell3, w1);
-                emit(t - 1, w0, w1);
-                copy(w0, w1);
+                b_half_store(t - 1, acc, w1);
+                a_half(w1, acc);
             } else {
-                emit(n3 - 1, w0, wfirst);
+                b_half_store(n3 - 1, acc, wfirst);
             }
         }
     }

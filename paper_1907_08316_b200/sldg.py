@@ -18,7 +18,7 @@ EXPORTS = [
     "sldg_create", "sldg_destroy", "sldg_last_error", "sldg_num_dofs", "sldg_num_x",
     "sldg_node_coords", "sldg_set_initial", "sldg_get_f", "sldg_current", "sldg_fill_uniform",
     "sldg_translate", "sldg_translate_dev", "sldg_advect", "sldg_advect_pair", "sldg_translate_pair_dev", "sldg_advect_triple", "sldg_translate_triple_dev", "sldg_compute_rho", "sldg_poisson_E",
-    "sldg_set_E", "sldg_step", "sldg_diagnostics", "sldg_moments", "sldg_launch_count",
+    "sldg_set_E", "sldg_step", "sldg_diagnostics", "sldg_moments", "sldg_invariants", "sldg_launch_count",
 ]
 
 
@@ -56,6 +56,7 @@ def _load():
     lib.sldg_step.argtypes = [vp, C.c_double]
     lib.sldg_diagnostics.argtypes = [vp, dp, dp, dp]
     lib.sldg_moments.argtypes = [vp, dp, dp]
+    lib.sldg_invariants.argtypes = [vp, dp, dp, dp, dp, dp]
     lib.sldg_launch_count.argtypes = [vp]
     lib.sldg_launch_count.restype = C.c_ulonglong
     return lib
@@ -231,6 +232,13 @@ class Sldg:
         k = C.c_double()
         self._chk(_lib.sldg_moments(self.h, P, C.byref(k)), "moments")
         return np.array(list(P)), k.value
+
+    def invariants(self):
+        """(mass, l2, electric energy, momentum[dv], kinetic energy) from one read of f."""
+        m, l2, ee, k = C.c_double(), C.c_double(), C.c_double(), C.c_double()
+        P = (C.c_double * self.dv)()
+        self._chk(_lib.sldg_invariants(self.h, C.byref(m), C.byref(l2), C.byref(ee), P, C.byref(k)), "invariants")
+        return m.value, l2.value, ee.value, np.array(list(P)), k.value
 
     def launch_count(self):
         return int(_lib.sldg_launch_count(self.h))

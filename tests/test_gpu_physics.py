@@ -166,6 +166,47 @@ def test_moments_match_oracle(oracle, shape, dtype):
     assert abs(K - Kr) <= 1e-13 * abs(Kr)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(1, 1, (9, 7)), (2, 2, (6, 5, 4, 7)), (3, 3, (4, 3, 5, 3, 4, 3)),
+                                   (1, 3, (8, 5, 4, 3)), (2, 2, (40, 36, 20, 24))])
+def test_invariants_one_read_of_f(oracle, shape, dtype):
+    """NEXT-4 as S:8(f) words it: mass, l2, electric energy, momentum and kinetic energy from ONE pass
+    over f (sldg_invariants), against the oracle; the result is remembered until f changes, so
+    diagnostics + moments + invariants on the same f launch the pass once, and a sweep invalidates it."""
+    dx, dv, cells = shape
+    o = 3 if dx < 3 else 2
+    lo = (0.0,) * dx + (-4.0, -3.0, -5.0)[:dv]
+    hi = tuple(2 * np.pi * (1 + 0.5 * a) for a in range(dx)) + (4.5, 3.5, 4.0)[:dv]
+    cfg = W.Config("inv", dx, dv, cells, o, lo, hi)
+    rng = np.random.default_rng(11)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
+    g = _grid(oracle, cfg)
+    s = make_solver(cfg, dtype)
+    s.set_initial(f0)
+    l0 = s.launch_count()
+    m, l2, ee, P, K = s.invariants()
+    first = s.launch_count() - l0
+    mr, l2r, eer = g.diagnostics(f0)
+    Pr, Kr = g.moments(f0)
+    assert abs(m - mr) <= 1e-13 * abs(mr) and abs(l2 - l2r) <= 1e-13 * abs(l2r)
+    assert abs(ee - eer) <= 1e-11 * abs(eer)
+    assert np.max(np.abs(P - Pr)) <= 1e-13 * np.max(np.abs(Pr)) + 1e-13 * abs(Kr)
+    assert abs(K - Kr) <= 1e-13 * abs(Kr)
+    # the same f again, through the two older calls: no kernel is launched, same numbers
+    l1 = s.launch_count()
+    assert s.diagnostics() == (m, l2, ee)
+    P2, K2 = s.moments()
+    assert s.launch_count() == l1 and K2 == K and np.array_equal(P2, P) and first > 0
+    # rho and E describe the current f after the pass (sldg.h)
+    assert rel_err(s.compute_rho().cpu().numpy(), g.rho(f0)) <= 1e-13
+    # a sweep invalidates the remembered result
+    s.advect(0, 0.05)
+    l2_ = s.launch_count()
+    m3 = s.invariants()[0]
+    assert s.launch_count() > l2_ and abs(m3 - m) <= TOL[dtype] * abs(m)    # mass is conserved (P5)
+    s.close()
+
+
 def test_config1_momentum_and_total_energy_on_the_gpu(oracle):
     cfg = W.CONFIG1
     s = make_solver(cfg, "f64")
