@@ -133,6 +133,14 @@ int sldg_poisson_E(sldg_ctx *ctx, double *E_device_or_null);
 /* Overwrite the stored E ([dx][X] fp64, host or device): lets a caller drive sldg_advect in v. */
 int sldg_set_E(sldg_ctx *ctx, const double *E, int is_device);
 
+/* S:8(f) NEXT-1: the x half-step and the density that follows it ("advection x", "compute rho") as ONE
+ * pass over f: sweeps x_1..x_dx with increment tau exactly as sldg_advect / _pair / _triple would (f is
+ * bit-identical), and leaves rho of the result in the context (and in rho_device_or_null, X doubles on the
+ * device, if not NULL).  When d_x = 2 or 3 and the fused sweep kernels apply, rho is accumulated while the
+ * last sweep writes f (no separate read of f); otherwise it is the sweeps followed by sldg_compute_rho.
+ * sldg_step uses this call for its first x half-step. */
+int sldg_advect_x_rho(sldg_ctx *ctx, double tau, double *rho_device_or_null);
+
 /* Strang step (D:O6 row a-5): x_1..x_dx with dt/2, rho, Poisson, v_1..v_dx with dt,
  * x_1..x_dx with dt/2. */
 int sldg_step(sldg_ctx *ctx, double dt);

@@ -51,6 +51,9 @@ struct sldg_ctx {
         int tile_pair = -1;            // SLDG_TILE_PAIR: -1 default (o >= 3), 0 never, 1 always
         bool tile_triple = true;       // SLDG_NO_TILE_TRIPLE=1 -> false
         int vt_variant = -1;           // SLDG_VTRIPLE_VARIANT: staged v-triple variant (-1 = default)
+        bool fuse_rho = true;          // SLDG_NO_FUSE_RHO=1 -> false: rho is a pass of its own after the x-group
+        bool rho_triple = false;       // SLDG_RHO_TRIPLE=1: also fuse rho into the x-triple (3+3 D: measured break-even, off)
+        int rho_cells = 0;             // SLDG_RHO_CELLS: cells per block range in the fused x-group + rho kernels (0 = default)
     } tune;
     // TMA descriptors depend only on (buffer, view), both fixed for the life of the context: encoded once
     struct TmapSlot { CUtensorMap map; bool valid = false; int p0 = 0, p1 = 0; };
@@ -109,6 +112,8 @@ struct sldg_ctx {
     bool use_fuse = true;              // SLDG_NO_FUSE=1: sldg_step issues one sweep per pass
     bool use_tma = true;               // SLDG_NO_TMA=1 in the environment selects the plain kernels
     bool have_rho = false, have_E = false;
+    bool want_rho = false;             // the next fused x-group sweep should also leave the rho partials (NEXT-1)
+    int rho_rows = 0;                  // > 0: that sweep left rho_rows partial rows [rho_rows][X] in d_part
     bool have_inv = false;             // d_part holds the one-read invariant partials of the CURRENT f
     unsigned long long launches = 0;
     char err[512] = "";
@@ -162,7 +167,7 @@ struct DeviceGuard {
 // opt in to `bytes` of dynamic shared memory for `kernel` on this context's device (once per size)
 template <typename K>
 cudaError_t ensure_smem(sldg_ctx *c, K kernel, size_t bytes) {
-    if (bytes <= 48 * 1024) return cudaSuccess;
+    if (bytes <= 32 * 1024) return cudaSuccess;          // static + dynamic must stay under the 48 KB default
     size_t &have = c->smem_attr[(const void *)kernel];
     if (bytes <= have) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
@@ -270,6 +275,9 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         c->tune.tile_triple = !env_flag("SLDG_NO_TILE_TRIPLE");
         c->tune.tile_pair = env_int("SLDG_TILE_PAIR", -1, 0, 1);
         c->tune.vt_variant = env_int("SLDG_VTRIPLE_VARIANT", -1, 0, 15);
+        c->tune.fuse_rho = !env_flag("SLDG_NO_FUSE_RHO");
+        c->tune.rho_triple = env_flag("SLDG_RHO_TRIPLE");
+        c->tune.rho_cells = env_int("SLDG_RHO_CELLS", 0, 1, 8);
         // columns per tile: a power of two in [8, 128] whose row is a multiple of 16 bytes; anything else is ignored
         int w = env_int("SLDG_TILE_W", 0, 8, 128);
         if (w > 0 && (w & (w - 1)) == 0 && (w * (int)c->esize) % 16 == 0) c->tune.tile_w = w;
@@ -630,6 +638,36 @@ int run_sweep(sldg_ctx *c, int dim, long count) {
 }
 
 // ---- fused pair of sweeps (sweep_fused.cuh); d_sigma / d_sigma2 hold the two shift tables ----
+// x_1 x_2 pair + rho (sweep_xpair_rho_kernel): ONE wave of equal blocks = (x_2-cell groups) x (plane chunks)
+template <typename T, int O, int C2R>
+int launch_xpair_rho(sldg_ctx *c, const T *in, T *out, int n1, int n2, long planes, long count1, long qd1, long qm1,
+                     long count2, long qd2, long qm2) {
+    const size_t slab_bytes = (size_t)O * n1 * O * sizeof(T);
+    const size_t slot = (slab_bytes + 127) & ~(size_t)127;
+    const size_t smem = 8 * slot;
+    auto kern = sweep_xpair_rho_kernel<T, O, C2R>;
+    // shift index of plane p: q_i = (p / pdiv_i) % pmod_i (a plane is X = qd1 elements when d_x = 2)
+    const long X = (long)n1 * O * n2 * O;
+    qd1 /= X; qd2 /= X;
+    CUDA_TRY(c, ensure_smem(c, kern, smem));
+    const int blk = (int)(cdiv(n1, 32) * 32);
+    int per_sm = 0;
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, blk, smem));
+    if (per_sm < 1) per_sm = 1;
+    const long G = cdiv(n2, C2R);
+    long nchunk = (long)c->sm_count * per_sm / G;
+    const long cap = (long)(3 + c->dv) * c->max_splits;
+    if (nchunk > cap) nchunk = cap;
+    if (nchunk > planes) nchunk = planes;
+    if (nchunk < 1) nchunk = 1;
+    kern<<<(unsigned)(nchunk * G), blk, smem, c->stream>>>(
+        in, out, n1, n2, planes, (int)nchunk, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2,
+        (const T *)c->d_ab2, count2, qd2, qm2, c->d_Wv, c->d_part);
+    LAUNCH_CHECK(c);
+    c->rho_rows = (int)nchunk;
+    return SLDG_OK;
+}
+
 template <typename T, int O>
 int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
     const int n1 = c->cells[k1], n2 = c->cells[k2];
@@ -674,6 +712,27 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
     long threads = lines * nseg;
     int chunk = 32;
     while (inner1 % chunk) chunk /= 2;
+    // x_1 x_2 (the whole x-group of a d_x = 2 step) with rho accumulated in the same pass
+    if (c->want_rho && c->use_tma && (O == 2 || O == 3 || c->tune.rho_cells) && k1 == 0 && k2 == 1 && c->dx == 2 && n1 <= 256 && n2 >= 2 &&
+        ((size_t)O * n1 * O * sizeof(T)) % 16 == 0 && 8 * (((size_t)O * n1 * O * sizeof(T) + 127) & ~(size_t)127) <= 96 * 1024) {
+        const long planes = midN * outer2;                   // = V
+        int cells = c->tune.rho_cells ? c->tune.rho_cells : (O == 1 ? 8 : 4);   // config 3: 4 cells 0.717 ms, 8 cells 0.822 ms (186 registers)
+        int rc = -1;
+        if constexpr (O <= 2) {
+            if (cells >= 8) rc = launch_xpair_rho<T, O, 8>(c, in, out, n1, n2, planes, count1, qd1, qm1, count2, qd2, qm2);
+            else if (cells >= 4) rc = launch_xpair_rho<T, O, 4>(c, in, out, n1, n2, planes, count1, qd1, qm1, count2, qd2, qm2);
+            else rc = launch_xpair_rho<T, O, 2>(c, in, out, n1, n2, planes, count1, qd1, qm1, count2, qd2, qm2);
+        } else if constexpr (O == 3) {
+            if (cells >= 4) rc = launch_xpair_rho<T, O, 4>(c, in, out, n1, n2, planes, count1, qd1, qm1, count2, qd2, qm2);
+            else rc = launch_xpair_rho<T, O, 2>(c, in, out, n1, n2, planes, count1, qd1, qm1, count2, qd2, qm2);
+        } else {
+            rc = launch_xpair_rho<T, O, 2>(c, in, out, n1, n2, planes, count1, qd1, qm1, count2, qd2, qm2);
+        }
+        if (rc) return rc;
+        c->cur ^= 1;
+        f_changed(c);
+        return SLDG_OK;
+    }
     // x_1 x_2: copy-engine staged plane kernel, one block per (x_1, x_2) plane
     {
         const size_t slab_bytes = (size_t)O * n1 * O * sizeof(T);
@@ -777,6 +836,49 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
             for (int d = 0; d < c->dx + ks[i]; ++d) qd[i] *= c->N[d];
             qm[i] = c->N[c->dx + ks[i]];
         } else { qd[i] = 1; qm[i] = c->X; }
+    }
+    // x_1 x_2 x_3 (the whole x-group of a d_x = 3 step) with rho accumulated in the same pass
+    // (config 5: 17.7 ms fused vs 12.0 + 5.3 ms -- the accumulators have to live in shared memory and the plane
+    //  kernel is bound by shared-memory wavefronts already; SLDG_RHO_TRIPLE=1 enables it)
+    if (c->want_rho && c->tune.rho_triple && c->use_tma && k1 == 0 && k2 == 1 && k3 == 2 && c->dx == 3 && (long)n1 * n2 <= 512 && n3 >= 2 &&
+        ((size_t)O * n2 * O * n1 * O * sizeof(T)) % 16 == 0) {
+        const size_t slab_bytes = (size_t)O * n2 * O * n1 * O * sizeof(T);
+        const size_t slot = (slab_bytes + 127) & ~(size_t)127;
+        const size_t slab_acc = (size_t)O * n2 * O * n1 * O * sizeof(double);
+        auto go = [&](auto kern, int C3R, int NS) -> int {
+            const size_t smem = NS * slot + C3R * slab_acc;
+            if (smem > 226 * 1024) return 1;
+            if (ensure_smem(c, kern, smem) != cudaSuccess) { cudaGetLastError(); return 1; }
+            const int blk = (int)(cdiv((long)n1 * n2, 32) * 32);
+            int per_sm = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, blk, smem) != cudaSuccess || per_sm < 1) {
+                cudaGetLastError();
+                return 1;
+            }
+            const long G = cdiv(n3, C3R);
+            long nchunk = (long)c->sm_count * per_sm / G;
+            const long cap = (long)(3 + c->dv) * c->max_splits;
+            if (nchunk > cap) nchunk = cap;
+            if (nchunk > outer3) nchunk = outer3;
+            if (nchunk < 1) nchunk = 1;
+            kern<<<(unsigned)(nchunk * G), blk, smem, c->stream>>>(
+                in, out, n1, n2, n3, outer3, (int)nchunk, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1],
+                (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2], c->d_Wv, c->d_part);
+            c->rho_rows = (int)nchunk;
+            return 0;
+        };
+        // range of x_3-cells per block: as many as fit beside a 3-deep ring (fewer cells = more neighbour slabs)
+        int rc = 1;
+        const int want = c->tune.rho_cells;
+        if (rc && (want == 0 || want == 5)) rc = go(sweep_xtriple_rho_kernel<T, O, 5, 3>, 5, 3);
+        if (rc && (want == 0 || want == 4)) rc = go(sweep_xtriple_rho_kernel<T, O, 4, 4>, 4, 4);
+        if (rc && (want == 0 || want == 2)) rc = go(sweep_xtriple_rho_kernel<T, O, 2, 4>, 2, 4);
+        if (rc == 0) {
+            LAUNCH_CHECK(c);
+            c->cur ^= 1;
+            f_changed(c);
+            return SLDG_OK;
+        }
     }
     // x_1 x_2 x_3 with a small x-grid: copy-engine staged plane kernel, one block per velocity node
     {
@@ -1232,9 +1334,14 @@ extern "C" int sldg_translate_triple_dev(sldg_ctx *c, int dim1, const double *sh
 }
 
 namespace {
-// sweeps along dimensions base .. base+cnt-1 with increment tau, fusing the first two when allowed
-int advect_group(sldg_ctx *c, int base, int cnt, double tau) {
+// sweeps along dimensions base .. base+cnt-1 with increment tau, fusing the first two when allowed;
+// with_rho: the fused kernel that performs the WHOLE group may also leave the rho partials (c->rho_rows)
+int advect_group(sldg_ctx *c, int base, int cnt, double tau, bool with_rho = false) {
     int rc, a = 0;
+    c->rho_rows = 0;
+    const bool whole = c->use_fuse && ((cnt == 3 && c->o <= 2) || (cnt == 2 && c->o <= 4));
+    c->want_rho = with_rho && whole && c->tune.fuse_rho && base == 0;
+    struct Clear { sldg_ctx *c; ~Clear() { c->want_rho = false; } } clear{c};
     if (c->use_fuse && cnt == 3 && c->o <= 2) return sldg_advect_triple(c, base, base + 1, base + 2, tau);
     if (c->use_fuse && cnt >= 2) {
         if ((rc = sldg_advect_pair(c, base, base + 1, tau))) return rc;
@@ -1246,10 +1353,21 @@ int advect_group(sldg_ctx *c, int base, int cnt, double tau) {
 }  // namespace
 
 namespace {
+// x-group with increment tau, then rho of the result: one pass when the fused kernels apply (NEXT-1)
+int advect_x_rho(sldg_ctx *c, double tau, double *rho_copy) {
+    int rc = advect_group(c, 0, c->dx, tau, true);
+    if (rc) return rc;
+    if (c->rho_rows > 0) {
+        const int rows = c->rho_rows;
+        c->rho_rows = 0;
+        return finish_vsum(c, rows, rho_copy, false);
+    }
+    return run_rho(c, rho_copy);
+}
+
 int step_body(sldg_ctx *c, double dt) {
     int rc;
-    if ((rc = advect_group(c, 0, c->dx, 0.5 * dt))) return rc;
-    if ((rc = run_rho(c, nullptr))) return rc;
+    if ((rc = advect_x_rho(c, 0.5 * dt, nullptr))) return rc;
     if ((rc = run_poisson(c, nullptr))) return rc;
     if ((rc = advect_group(c, c->dx, c->dx, dt))) return rc;
     if ((rc = advect_group(c, 0, c->dx, 0.5 * dt))) return rc;
@@ -1290,6 +1408,12 @@ int capture_step(sldg_ctx *c, double dt, sldg_ctx::StepGraph &g) {
     return SLDG_OK;
 }
 }  // namespace
+
+extern "C" int sldg_advect_x_rho(sldg_ctx *c, double tau, double *rho_out) {
+    if (!c) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
+    return advect_x_rho(c, tau, rho_out);
+}
 
 extern "C" int sldg_step(sldg_ctx *c, double dt) {
     if (!c) return SLDG_ERR_ARG;

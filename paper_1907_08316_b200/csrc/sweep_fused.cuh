@@ -1034,3 +1034,387 @@ sweep_vtriple_tile_kernel(const __grid_constant__ CUtensorMap tmap, const T *__r
 }
 
 }  // namespace sldg
+
+namespace sldg {
+
+// ------------------------------------------------------------------------------------------
+// S:8(f) NEXT-1, the rest of it: rho ACCUMULATED IN THE SWEEP THAT PRECEDES IT ("compute rho" follows the
+// x half-step).  x_1 x_2 pair + rho for d_x = 2.
+//
+// sweep_xpair_plane_kernel gives one block a whole (x_1,x_2) plane at fixed v; summing over v inside the
+// kernel needs accumulators for every x-node a thread writes.  Here a block owns a RANGE of C2R x_2-cells
+// (group g) and walks a contiguous chunk of planes (velocity nodes, the slow index): thread c1 keeps
+// C2R * O * O fp64 accumulators (fp64 for both storage types) for its x-nodes and adds W_v * f_new
+// plane after plane in ascending v -- the split structure of the stand-alone rho pass with chunks as splits.
+// Per plane the block streams the C2R + 1 slabs (k2-cells) its outputs need -- the extra one is the k2
+// neighbour, an L2 hit for the group next door -- through the same cp.async.bulk ring, which never drains
+// between planes.  The grid is ONE wave of equal blocks (groups x chunks = resident blocks), so the
+// partials part[chunk][x] are a fraction (chunks / V) of one write of f and the order of every sum is fixed.
+// f is bit-identical to the two separate sweeps; rho = -(pass over the chunks) as in vsum_final_kernel.
+// ------------------------------------------------------------------------------------------
+template <typename T, int O, int C2R>
+__global__ void __launch_bounds__(256)
+sweep_xpair_rho_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2, long planes, int nchunk,
+                       const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long pdiv1, long pmod1,
+                       const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long pdiv2, long pmod2,
+                       const double *__restrict__ Wv, double *__restrict__ part) {
+    // shift index of plane p (a velocity node): q_i = (p / pdiv_i) % pmod_i, kept incrementally (no divisions
+    // in the loops: thread 0's producer path holds up the whole block at the next barrier)
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    constexpr int NS = 8;                                   // ring depth
+    constexpr int NCO = 4 * O * O;                           // A1 | B1 | A2 | B2
+    __shared__ __align__(8) uint64_t full[NS];
+    __shared__ T s_co[2][NCO];                               // coefficients of the current / next plane
+    __shared__ int s_m1[2];
+    __shared__ double s_wv[2];
+    const long N1 = (long)n1 * O;
+    const long slab = O * N1;                                // elements per k2-cell of one plane
+    const uint32_t slab_bytes = (uint32_t)((size_t)slab * sizeof(T));
+    const uint32_t slot_stride = (slab_bytes + 127u) & ~127u;
+    const int G = (n2 + C2R - 1) / C2R;
+    const int g = blockIdx.x % G;
+    const long chunk = blockIdx.x / G;
+    const long p0 = chunk * planes / nchunk, p1 = (chunk + 1) * planes / nchunk;
+    const int i0 = g * C2R;                                  // first owned k2-cell
+    const int ncell = (n2 - i0 < C2R) ? n2 - i0 : C2R;       // owned cells (ragged last group)
+    const int L = ncell + 1;                                 // slabs per plane
+    const long total = (p1 - p0) * L;
+    const int tid = threadIdx.x;
+    const int c1 = tid;
+    const bool active = c1 < n1;
+    const long plane_elems = (long)n2 * slab;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+    }
+    // consumer counters of plane p0
+    long q1 = (p0 / pdiv1) % pmod1, r1 = p0 % pdiv1, q2 = (p0 / pdiv2) % pmod2, r2 = p0 % pdiv2;
+    auto fetch_coef = [&](int e, long qa, long qb) -> T {    // element e of [A1 | B1 | A2 | B2] of a plane
+        return e < 2 * O * O ? ab1[(long)e * count1 + qa] : ab2[(long)(e - 2 * O * O) * count2 + qb];
+    };
+    for (int e = tid; e < NCO; e += blockDim.x) s_co[0][e] = fetch_coef(e, q1, q2);
+    if (tid == 0) { s_m1[0] = mtab1[q1]; s_wv[0] = p0 < p1 ? Wv[p0] : 0.0; }
+    __syncthreads();
+    // producer state (thread 0): next slab to issue = slab kp of plane ip; m2 of that plane and of the next
+    long ip = p0, pq2 = q2, pr2 = r2;
+    int kp = 0, pslot = 0;
+    long issued = 0;
+    int m2p = 0, m2n = 0;
+    if (tid == 0) m2n = mtab2[pq2];
+    auto issue = [&]() {
+        if (kp == 0) {                                       // entering plane ip: its m2 was fetched a plane ago
+            m2p = m2n;
+            if (++pr2 == pdiv2) { pr2 = 0; if (++pq2 == pmod2) pq2 = 0; }
+            m2n = mtab2[pq2];
+        }
+        int cell = i0 + m2p + kp;
+        if (cell >= n2) cell -= n2;
+        if (cell >= n2) cell -= n2;
+        mbar_expect_tx(&full[pslot], slab_bytes);
+        bulk_g2s(smem_raw + pslot * slot_stride, in + ip * plane_elems + (long)cell * slab, slab_bytes, &full[pslot]);
+        ++issued;
+        if (++pslot == NS) pslot = 0;
+        if (++kp == L) { kp = 0; ++ip; }
+    };
+    if (tid == 0)
+        for (int j = 0; j < NS && j < total; ++j) issue();
+
+    double racc[C2R][O][O];
+#pragma unroll
+    for (int a = 0; a < C2R; ++a)
+#pragma unroll
+        for (int b = 0; b < O; ++b)
+#pragma unroll
+            for (int d = 0; d < O; ++d) racc[a][b][d] = 0.0;
+
+    int slot = 0;
+    uint32_t phase = 0;
+    T *dst_plane = out + p0 * plane_elems + (long)i0 * slab + (long)c1 * O;
+    for (long pl = p0; pl < p1; ++pl) {
+        const int buf = (int)((pl - p0) & 1);
+        T A1[O * O], B1[O * O], A2[O * O], B2[O * O];
+#pragma unroll
+        for (int e = 0; e < O * O; ++e) {
+            A1[e] = s_co[buf][e]; B1[e] = s_co[buf][O * O + e];
+            A2[e] = s_co[buf][2 * O * O + e]; B2[e] = s_co[buf][3 * O * O + e];
+        }
+        const int m1 = s_m1[buf];
+        const double wv = s_wv[buf];
+        // next plane's coefficients: loads issued now, stored to the other buffer before the plane's last barrier
+        if (++r1 == pdiv1) { r1 = 0; if (++q1 == pmod1) q1 = 0; }
+        if (++r2 == pdiv2) { r2 = 0; if (++q2 == pmod2) q2 = 0; }
+        const bool more = pl + 1 < p1;
+        T pre = T(0);
+        int pre_m = 0;
+        double pre_w = 0.0;
+        if (more) {
+            if (tid < NCO) pre = fetch_coef(tid, q1, q2);
+            if (tid == 0) { pre_m = mtab1[q1]; pre_w = Wv[pl + 1]; }
+        }
+        int sa1 = (active ? c1 : 0) + m1; if (sa1 >= n1) sa1 -= n1;
+        int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
+        const int oa = sa1 * O, ob = sb1 * O;
+        T acc[O][O];                                         // A-half of the k2 rule on the older cell
+#pragma unroll
+        for (int k = 0; k <= C2R; ++k) {
+            if (k < L) {
+                mbar_wait(&full[slot], phase);
+                T w[O][O];                                   // k1-swept values of this thread's cell, w[l2][j1]
+                if (active) {
+                    const T *sl = reinterpret_cast<const T *>(smem_raw + slot * slot_stride);
+#pragma unroll
+                    for (int l2 = 0; l2 < O; ++l2) {
+                        T r0[O], r1v[O];
+                        load_cell<T, O>(sl + l2 * N1 + oa, r0);
+                        load_cell<T, O>(sl + l2 * N1 + ob, r1v);
+#pragma unroll
+                        for (int j1 = 0; j1 < O; ++j1) w[l2][j1] = chain<T, O>(A1, B1, j1, r0, r1v);
+                    }
+                }
+                if (k == L - 1 && more) {                    // hand the next plane's coefficients over
+                    if (tid < NCO) s_co[buf ^ 1][tid] = pre;
+                    if constexpr (NCO > 32) {                // blocks may be as small as one warp
+                        for (int e = tid + blockDim.x; e < NCO; e += blockDim.x) s_co[buf ^ 1][e] = fetch_coef(e, q1, q2);
+                    }
+                    if (tid == 0) { s_m1[buf ^ 1] = pre_m; s_wv[buf ^ 1] = pre_w; }
+                }
+                __syncthreads();                             // slab consumed: refill the slot before the k2 rule
+                if (tid == 0 && issued < total) issue();
+                if (++slot == NS) { slot = 0; phase ^= 1u; }
+                if (active) {
+                    if (k > 0) {                             // B-half, store, rho
+                        T *dst = dst_plane + (long)(k - 1) * slab;
+#pragma unroll
+                        for (int j2 = 0; j2 < O; ++j2) {
+                            T res[O];
+#pragma unroll
+                            for (int j1 = 0; j1 < O; ++j1) {
+                                T a = acc[j2][j1];
+#pragma unroll
+                                for (int l = 0; l < O; ++l) a = fma_t<T>(B2[j2 * O + l], w[l][j1], a);
+                                res[j1] = a;
+                                racc[k > 0 ? k - 1 : 0][j2][j1] += wv * (double)a;
+                            }
+                            T *p = dst + (long)j2 * N1;
+                            if constexpr (O % 2 == 0) {
+                                using V2 = Vec<T, 2>;
+#pragma unroll
+                                for (int j1 = 0; j1 < O; j1 += 2) {
+                                    V2 vv; vv.v[0] = res[j1]; vv.v[1] = res[j1 + 1];
+                                    *reinterpret_cast<V2 *>(p + j1) = vv;
+                                }
+                            } else {
+#pragma unroll
+                                for (int j1 = 0; j1 < O; ++j1) p[j1] = res[j1];
+                            }
+                        }
+                    }
+                    if (k < C2R) {                           // A-half for the next cell
+#pragma unroll
+                        for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                            for (int j1 = 0; j1 < O; ++j1) {
+                                T a = mul_t<T>(A2[j2 * O], w[0][j1]);
+#pragma unroll
+                                for (int l = 1; l < O; ++l) a = fma_t<T>(A2[j2 * O + l], w[l][j1], a);
+                                acc[j2][j1] = a;
+                            }
+                    }
+                }
+            }
+        }
+        dst_plane += plane_elems;
+    }
+    if (active) {
+        double *pr = part + chunk * plane_elems;             // row `chunk` of [nchunk][X], X = n2 * slab
+#pragma unroll
+        for (int k = 0; k < C2R; ++k)
+            if (k < ncell)
+#pragma unroll
+                for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1)
+                        pr[((long)(i0 + k) * O + j2) * N1 + (long)c1 * O + j1] = racc[k][j2][j1];
+    }
+}
+
+}  // namespace sldg
+
+namespace sldg {
+
+// ------------------------------------------------------------------------------------------
+// x_1 x_2 x_3 triple + rho for d_x = 3 with a small x-grid (the 3+3 D step): sweep_xtriple_plane_kernel with
+// the v-sum inside.  A block owns a range of C3R x_3-cells (group g) and walks a contiguous chunk of
+// velocity nodes; per node it streams the C3R + 1 slabs (x_3-cells, each one contiguous O * N2 * N1 values)
+// its outputs need through the cp.async.bulk ring.  The accumulators -- C3R * O^3 fp64 per thread -- do not
+// fit the register file next to the O^3 window and the six A,B matrices, so they live in SHARED memory, each
+// word owned by exactly one thread (no atomics, fixed order: ascending v).  One wave of equal blocks; the
+// partials part[chunk][x] are chunks / V of one write of f.  f is bit-identical to the three sweeps.
+// ------------------------------------------------------------------------------------------
+template <typename T, int O, int C3R, int NS>
+__global__ void __launch_bounds__(512, 1)
+sweep_xtriple_rho_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2, int n3, long nv, int nchunk,
+                         const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
+                         const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2,
+                         const int *__restrict__ mtab3, const T *__restrict__ ab3, long count3, long qdiv3, long qmod3,
+                         const double *__restrict__ Wv, double *__restrict__ part) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t full[NS];
+    const long N1 = (long)n1 * O, N2 = (long)n2 * O;
+    const long slab = O * N2 * N1;                           // elements per k3-cell
+    const size_t slab_bytes = (size_t)slab * sizeof(T);
+    const size_t slot_stride = (slab_bytes + 127) & ~(size_t)127;
+    double *racc = reinterpret_cast<double *>(smem_raw + NS * slot_stride);   // [C3R][slab]
+    const int G = (n3 + C3R - 1) / C3R;
+    const int g = blockIdx.x % G;
+    const long chunk = blockIdx.x / G;
+    const long v0 = chunk * nv / nchunk, v1 = (chunk + 1) * nv / nchunk;
+    const int i0 = g * C3R;
+    const int ncell = (n3 - i0 < C3R) ? n3 - i0 : C3R;
+    const int L = ncell + 1;
+    const long total = (v1 - v0) * L;
+    const int tid = threadIdx.x;
+    const int c1 = tid % n1, c2 = tid / n1;
+    const bool active = c2 < n2;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+    }
+    for (long e = tid; e < (long)C3R * slab; e += blockDim.x) racc[e] = 0.0;
+    __syncthreads();
+    long ip = v0;
+    int kp = 0, m3p = 0, m3n = 0;
+    long issued = 0;
+    if (tid == 0 && v0 < v1) m3n = mtab3[((v0 * n3 * slab) / qdiv3) % qmod3];
+    auto issue = [&]() {
+        if (kp == 0) {                                       // m3 of node ip was fetched a node ago
+            m3p = m3n;
+            m3n = mtab3[(((ip + 1 < nv ? ip + 1 : ip) * n3 * slab) / qdiv3) % qmod3];
+        }
+        int cell = i0 + m3p + kp;
+        if (cell >= n3) cell -= n3;
+        if (cell >= n3) cell -= n3;
+        const int slot = (int)(issued % NS);
+        mbar_expect_tx(&full[slot], (uint32_t)slab_bytes);
+        bulk_g2s(smem_raw + slot * slot_stride, in + (ip * n3 + cell) * slab, (uint32_t)slab_bytes, &full[slot]);
+        ++issued;
+        if (++kp == L) { kp = 0; ++ip; }
+    };
+    if (tid == 0)
+        for (int j = 0; j < NS && j < total; ++j) issue();
+
+    int slot = 0;
+    uint32_t phase = 0;
+    for (long v = v0; v < v1; ++v) {
+        const long base = v * (long)n3 * slab;
+        const long q1 = (base / qdiv1) % qmod1, q2 = (base / qdiv2) % qmod2, q3 = (base / qdiv3) % qmod3;
+        T A1[O * O], B1[O * O], A2[O * O], B2[O * O], A3[O * O], B3[O * O];
+#pragma unroll
+        for (int e = 0; e < O * O; ++e) {
+            A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1];
+            A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
+            A3[e] = ab3[(long)e * count3 + q3]; B3[e] = ab3[(long)(O * O + e) * count3 + q3];
+        }
+        const int m1 = mtab1[q1], m2 = mtab2[q2];
+        const double wv = Wv[v];
+        int sa1 = c1 + m1; if (sa1 >= n1) sa1 -= n1;
+        int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
+        int sa2 = (active ? c2 : 0) + m2; if (sa2 >= n2) sa2 -= n2;
+        int sb2 = sa2 + 1; if (sb2 == n2) sb2 = 0;
+        const int off[2][2] = {{(int)(sa2 * O * N1 + sa1 * O), (int)(sa2 * O * N1 + sb1 * O)},
+                               {(int)(sb2 * O * N1 + sa1 * O), (int)(sb2 * O * N1 + sb1 * O)}};
+        T acc[O][O][O];                                      // A-half of the k3 rule on the older cell
+#pragma unroll 1
+        for (int k = 0; k < L; ++k) {
+            mbar_wait(&full[slot], phase);
+            T w[O][O][O];                                    // (k1,k2)-swept values of this thread's cell pair
+            if (active) {
+                const T *sl = reinterpret_cast<const T *>(smem_raw + slot * slot_stride);
+#pragma unroll
+                for (int l3 = 0; l3 < O; ++l3) {
+                    T tk[2][O][O];
+#pragma unroll
+                    for (int e2 = 0; e2 < 2; ++e2)
+#pragma unroll
+                        for (int l2 = 0; l2 < O; ++l2) {
+                            T r0[O], r1[O];
+                            load_cell<T, O>(sl + l3 * N2 * N1 + off[e2][0] + l2 * N1, r0);
+                            load_cell<T, O>(sl + l3 * N2 * N1 + off[e2][1] + l2 * N1, r1);
+#pragma unroll
+                            for (int j1 = 0; j1 < O; ++j1) tk[e2][l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+                        }
+#pragma unroll
+                    for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                        for (int j1 = 0; j1 < O; ++j1) {
+                            T a0[O], a1[O];
+#pragma unroll
+                            for (int l = 0; l < O; ++l) { a0[l] = tk[0][l][j1]; a1[l] = tk[1][l][j1]; }
+                            w[l3][j2][j1] = chain<T, O>(A2, B2, j2, a0, a1);
+                        }
+                }
+            }
+            __syncthreads();                                 // slab consumed: refill the slot before the k3 rule
+            if (tid == 0 && issued < total) issue();
+            if (++slot == NS) { slot = 0; phase ^= 1u; }
+            if (active) {
+                if (k > 0) {                                 // B-half, store, rho
+                    const long cell_off = (long)c2 * O * N1 + (long)c1 * O;
+                    T *dst = out + base + (long)(i0 + k - 1) * slab + cell_off;
+                    double *ra = racc + (long)(k - 1) * slab + cell_off;
+#pragma unroll
+                    for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+                        for (int j2 = 0; j2 < O; ++j2) {
+                            T res[O];
+#pragma unroll
+                            for (int j1 = 0; j1 < O; ++j1) {
+                                T a = acc[j3][j2][j1];
+#pragma unroll
+                                for (int l = 0; l < O; ++l) a = fma_t<T>(B3[j3 * O + l], w[l][j2][j1], a);
+                                res[j1] = a;
+                            }
+                            const long ro = (long)j3 * N2 * N1 + (long)j2 * N1;
+                            T *p = dst + ro;
+                            double *pa = ra + ro;
+                            if constexpr (O % 2 == 0) {
+                                using V2 = Vec<T, 2>;
+                                using D2 = Vec<double, 2>;
+#pragma unroll
+                                for (int j1 = 0; j1 < O; j1 += 2) {
+                                    V2 vv; vv.v[0] = res[j1]; vv.v[1] = res[j1 + 1];
+                                    *reinterpret_cast<V2 *>(p + j1) = vv;
+                                    D2 r = *reinterpret_cast<D2 *>(pa + j1);
+                                    r.v[0] += wv * (double)res[j1]; r.v[1] += wv * (double)res[j1 + 1];
+                                    *reinterpret_cast<D2 *>(pa + j1) = r;
+                                }
+                            } else {
+#pragma unroll
+                                for (int j1 = 0; j1 < O; ++j1) { p[j1] = res[j1]; pa[j1] += wv * (double)res[j1]; }
+                            }
+                        }
+                }
+                if (k + 1 < L) {                             // A-half for the next cell
+#pragma unroll
+                    for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+                        for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                            for (int j1 = 0; j1 < O; ++j1) {
+                                T a = mul_t<T>(A3[j3 * O], w[0][j2][j1]);
+#pragma unroll
+                                for (int l = 1; l < O; ++l) a = fma_t<T>(A3[j3 * O + l], w[l][j2][j1], a);
+                                acc[j3][j2][j1] = a;
+                            }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    double *pr = part + chunk * (long)n3 * slab + (long)i0 * slab;     // row `chunk` of [nchunk][X], X = n3 * slab
+    for (long e = tid; e < (long)ncell * slab; e += blockDim.x) pr[e] = racc[e];
+}
+
+}  // namespace sldg

@@ -207,6 +207,49 @@ def test_invariants_one_read_of_f(oracle, shape, dtype):
     s.close()
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("cells_env", ["", "2", "4", "5", "8"])
+@pytest.mark.parametrize("shape", [(2, 2, (16, 16, 6, 5), 2), (2, 2, (12, 9, 5, 4), 3), (2, 2, (8, 7, 4, 3), 4),
+                                   (2, 2, (8, 3, 4, 3), 1), (3, 3, (6, 5, 7, 3, 4, 3), 2), (3, 3, (4, 4, 11, 3, 3, 2), 1),
+                                   (2, 3, (8, 8, 3, 4, 3), 2), (1, 1, (16, 12), 3), (3, 3, (4, 4, 4, 3, 3, 3), 3)])
+def test_advect_x_rho_is_the_sweeps_plus_rho(oracle, monkeypatch, shape, cells_env, dtype):
+    """NEXT-1 remainder: rho accumulated in the x-group sweep (sldg_advect_x_rho).  f must be bit-identical to
+    the x-group issued through sldg_advect_pair / _triple / sldg_advect, rho within 1e-13 of the oracle's rho
+    of that f; every block-range size (SLDG_RHO_CELLS), ragged cell counts, all orders the fused kernels take
+    and the shapes that fall back to the separate rho pass."""
+    dx, dv, cells, o = shape
+    if cells_env:
+        monkeypatch.setenv("SLDG_RHO_CELLS", cells_env)
+    monkeypatch.setenv("SLDG_RHO_TRIPLE", "1")        # the 3+3 D variant is off by default (break-even), tested all the same
+    lo = (0.0,) * dx + (-4.0, -3.0, -5.0)[:dv]
+    hi = tuple(2 * np.pi * (1 + 0.5 * a) for a in range(dx)) + (4.5, 3.5, 4.0)[:dv]
+    cfg = W.Config("xr", dx, dv, cells, o, lo, hi)
+    rng = np.random.default_rng(21)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
+    g = _grid(oracle, cfg)
+    tau = 0.37
+    a = make_solver(cfg, dtype)
+    a.set_initial(f0)
+    rho = a.advect_x_rho(tau).cpu().numpy()
+    fa = a.get_f()
+    b = make_solver(cfg, dtype)
+    b.set_initial(f0)
+    if dx == 3 and o <= 2:
+        b.advect_triple(0, 1, 2, tau)
+    elif dx == 2 and o <= 4:
+        b.advect_pair(0, 1, tau)
+    else:
+        for d in range(dx):
+            b.advect(d, tau)
+    fb = b.get_f()
+    assert np.array_equal(fa, fb)
+    assert rel_err(rho, g.rho(fb)) <= 1e-13
+    # the context's rho is that rho: Poisson may follow directly
+    E = a.poisson_E().cpu().numpy()
+    assert rel_err(E, g.poisson_E(g.rho(fb))) <= 1e-12
+    a.close(); b.close()
+
+
 def test_config1_momentum_and_total_energy_on_the_gpu(oracle):
     cfg = W.CONFIG1
     s = make_solver(cfg, "f64")

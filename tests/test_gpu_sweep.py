@@ -219,8 +219,11 @@ def test_fused_pair_rejects_mixed_groups():
 def test_step_fused_equals_step_unfused_bitwise(monkeypatch):
     cfg = W.CONFIG3.scaled((10, 8, 12, 6))
     outs = []
-    for flag in ("0", "1"):
+    # sweep fusion is bitwise neutral; rho accumulated in the x-sweep sums in another (fixed) grouping, so that
+    # variant (the default) is compared at rounding level
+    for flag, norho in (("0", "1"), ("1", "1"), ("0", "0")):
         monkeypatch.setenv("SLDG_NO_FUSE", flag)
+        monkeypatch.setenv("SLDG_NO_FUSE_RHO", norho)
         s = make_solver(cfg, "f64")
         coords = [s.node_coords(d) for d in range(4)]
         s.set_initial(W.initial_state(cfg, coords))
@@ -231,6 +234,8 @@ def test_step_fused_equals_step_unfused_bitwise(monkeypatch):
         s.close()
     assert np.array_equal(outs[0][0], outs[1][0])
     assert outs[0][1] < outs[1][1]             # the fused step really launches fewer sweeps
+    assert rel_err(outs[2][0], outs[0][0]) <= 1e-13
+    assert outs[2][1] < outs[0][1]             # ... and with rho inside the x-sweep one kernel fewer per step
 
 
 @pytest.mark.parametrize("o", [1, 2, 3, 4, 5, 6])
@@ -293,8 +298,11 @@ def test_fused_triple_is_bitwise_the_three_sweeps_3p3(oracle, o, dtype):
 def test_step_3p3_fused_equals_unfused_bitwise(monkeypatch):
     cfg = W.CONFIG5.scaled((6, 5, 4, 6, 4, 5))
     outs = []
-    for flag in ("0", "1"):
+    # sweep fusion is bitwise neutral; rho accumulated in the x-sweep sums in another (fixed) grouping, so that
+    # variant (the default) is compared at rounding level
+    for flag, norho in (("0", "1"), ("1", "1"), ("0", "0")):
         monkeypatch.setenv("SLDG_NO_FUSE", flag)
+        monkeypatch.setenv("SLDG_NO_FUSE_RHO", norho)
         s = make_solver(cfg, "f64")
         coords = [s.node_coords(d) for d in range(6)]
         s.set_initial(W.initial_state(cfg, coords))
