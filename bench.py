@@ -67,7 +67,7 @@ class ClockSampler:
         except Exception:
             self.proc = None
 
-    def stop(self):
+    def stop(self, full=False):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
         if self.proc is None:
             return out
@@ -95,6 +95,8 @@ class ClockSampler:
         if sm:
             out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
                    "samples": len(sm)}
+            if full:
+                out["sm_mhz_min"] = float(min(sm)); out["sm_mhz_peak"] = float(max(sm))
         return out
 
 
@@ -173,6 +175,57 @@ def choose_oracle_sample(total_steps, budget_s=120.0):
         if est <= budget_s:
             return cfg
     return W.CONFIG4.scaled((16, 16, 8, 8))
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+_ONE_THREAD_SNIPPET = r"""
+import sys, time, numpy as np
+sys.path.insert(0, %r)
+from oracle import sldg_oracle as O
+from paper_1907_08316_b200 import workloads as W
+cfg = W.CONFIG4.scaled((32, 32, 16, 16))
+f = np.random.default_rng(0).random(cfg.ndof)
+D = cfg.dx + cfg.dv
+t = 0.0
+for d in range(D):
+    sig = W.config4_shifts(cfg, d)
+    dep = [cfg.dx + d] if d < cfg.dx else list(range(cfg.dx))
+    t0 = time.perf_counter(); O.translate(f, cfg.N, cfg.order, d, sig, dep); t += time.perf_counter() - t0
+print(O.num_threads(), cfg.ndof * D / t)
+"""
+
+
+def oracle_one_thread():
+    """The same oracle with OMP_NUM_THREADS=1 on a small twin (one sweep per direction): DOF updates/s."""
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        out = subprocess.run([sys.executable, "-c", _ONE_THREAD_SNIPPET % ROOT], env=env, capture_output=True,
+                             text=True, timeout=120).stdout.split()
+        return {"threads": int(out[0]), "dof_updates_per_s": float(out[1]),
+                "value": 2.0 * 8 * float(out[1]) / 1e9, "unit": UNIT,
+                "sample": "one sweep per direction, config-4 recipe, cells=(32, 32, 16, 16)"}
+    except Exception as exc:
+        return {"error": str(exc)}
+
+
+def oracle_config3_step():
+    """One full-size Strang step of config 3 by the oracle (seconds), S:8(d)."""
+    from oracle import sldg_oracle as O
+    cfg = W.CONFIG3
+    g = O.Grid(cfg.dx, cfg.dv, cfg.cells, cfg.order, cfg.lo, cfg.hi)
+    f = W.initial_state(cfg, [g.coords(d) for d in range(cfg.dx + cfg.dv)])
+    t0 = time.perf_counter()
+    g.step(f, cfg.dt)
+    return time.perf_counter() - t0
 
 
 def run_reference(args):
@@ -269,13 +322,22 @@ def strang_step_table(torch, Sldg, cfg, dtype, steps):
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
+    launches_per_step = (s.launch_count() - l0) / steps
+    # the paper's own loop writes the invariants once per step: one more read of f (sldg_invariants)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        s.step(cfg.dt)
+        s.invariants()
+    torch.cuda.synchronize()
+    ms_inv = 1e3 * (time.perf_counter() - t0) / steps
     es = 8 if dtype == "f64" else 4
     passes = 2 * (3 * cfg.dx) + 1
     mass, l2, ee = s.diagnostics()
-    out = {"ms_per_step": ms, "passes_paper_accounting": passes,
+    out = {"ms_per_step": ms, "ms_per_step_with_invariants_every_step": ms_inv, "passes_paper_accounting": passes,
+           "gbs_paper_eq1_style_with_invariants": (passes + 1) * cfg.ndof * es / ms_inv / 1e6,
            "gbs_paper_eq1_style": passes * cfg.ndof * es / ms / 1e6,
            "dof_updates_per_s": 3 * cfg.dx * cfg.ndof / ms * 1e3,
-           "launches_per_step": (s.launch_count() - l0) / steps, "mass": mass, "electric_energy": ee}
+           "launches_per_step": launches_per_step, "mass": mass, "electric_energy": ee}
     s.close()
     del s
     torch.cuda.empty_cache()
@@ -395,6 +457,26 @@ def run_ours(args):
         "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
     }
 
+    # ---- per-direction SM clock (min / median / max) while that direction's sweep runs alone, S:8(d)
+    if world == 1:
+        pdc = {}
+        for d in range(D):
+            smp = ClockSampler(local)
+            torch.cuda.synchronize()
+            smp.start()
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            nrep = 40
+            e0.record()
+            for _ in range(nrep):
+                s.translate(d, shifts[d])
+            e1.record()
+            torch.cuda.synchronize()
+            ck = smp.stop(full=True)
+            pdc["dim%d" % d] = {"sm_mhz_min": ck.get("sm_mhz_min"), "sm_mhz": ck.get("sm_mhz"),
+                                "sm_mhz_max": ck.get("sm_mhz_peak"), "reasons": ck.get("reasons"),
+                                "gbs_alone": sweep_bytes * nrep / e0.elapsed_time(e1) / 1e6}
+        roofline["per_direction_clocks"] = pdc
+
     # ---- e2e: the same step through the C-ABI with HOST buffers (pinned), copies inside the timing
     if rank == 0 or world > 1:
         nbytes = cfg.ndof * es
@@ -464,7 +546,14 @@ def run_ours(args):
             "value": 2.0 * ocfg.ndof * es * D * nrep / t_sw / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
             "dof_updates_per_s": ocfg.ndof * D * nrep / t_sw,
             "per_direction_gbs": {"dim%d" % d: 2.0 * ocfg.ndof * es * nrep / t / 1e9 for d, t in ostep.per_dim.items()},
-            "sample": "%d bench step(s) of the config-4 recipe on reduced twin cells=%s (%.2e DOF)" % (nrep, ocfg.cells, ocfg.ndof)}
+            "sample": "%d bench step(s) of the config-4 recipe on reduced twin cells=%s (%.2e DOF)" % (nrep, ocfg.cells, ocfg.ndof),
+            "cpu_model": cpu_model(), "one_thread": oracle_one_thread()}
+        try:        # S:8(d): the oracle's full-size config-3 Strang step beside the library's
+            t_or = oracle_config3_step()
+            gpu_ms = line.get("strang_steps_fused", {}).get(W.CONFIG3.name, {}).get("ms_per_step")
+            line["cpu_baseline"]["config3_step"] = {"oracle_ms": 1e3 * t_or, "gpu_ms": gpu_ms, "cores": cores}
+        except Exception as exc:
+            line["cpu_baseline"]["config3_step"] = {"error": str(exc)}
 
     if rank == 0:
         print(json.dumps(line))

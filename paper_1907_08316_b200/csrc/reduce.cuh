@@ -150,18 +150,30 @@ scalars_kernel(const double *__restrict__ rho, const double *__restrict__ s2,
 
 namespace sldg {
 
-// out[k] = sum_x W_x sum_split part[k][split][x], k < nk (one block of 1024 threads, fixed order)
+// rows[k][x] = sum_split part[k][split][x], k < nk: one WARP per (k, x), lane l adds splits l, l+32, ... in
+// ascending order, then a fixed shuffle tree (as vsum_final_kernel; a single block walking splits * X * nk
+// values serially took milliseconds at X = 128, V = 2.4e6)
+__global__ void __launch_bounds__(256)
+vrows_final_kernel(const double *__restrict__ part, long X, int splits, int nsplit_cap, int nk,
+                   double *__restrict__ rows) {
+    const long w = ((long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (w >= (long)nk * X) return;
+    const long k = w / X, x = w - k * X;
+    double a = 0.0;
+    for (int s = lane; s < splits; s += 32) a += part[(k * nsplit_cap + s) * X + x];
+    a = warp_sum(a);
+    if (lane == 0) rows[k * X + x] = a;
+}
+
+// out[k] = sum_x W_x rows[k][x], k < nk (one block of 1024 threads, fixed order)
 __global__ void __launch_bounds__(1024)
-moments_final_kernel(const double *__restrict__ part, const double *__restrict__ Wx, long X, int splits,
-                     int nsplit_cap, int nk, double *__restrict__ out) {
+moments_final_kernel(const double *__restrict__ rows, const double *__restrict__ Wx, long X, int nk,
+                     double *__restrict__ out) {
     __shared__ double sm[32];
     for (int k = 0; k < nk; ++k) {
         double a = 0.0;
-        for (long x = threadIdx.x; x < X; x += blockDim.x) {
-            double s = 0.0;
-            for (int sp = 0; sp < splits; ++sp) s += part[((long)k * nsplit_cap + sp) * X + x];
-            a += Wx[x] * s;
-        }
+        for (long x = threadIdx.x; x < X; x += blockDim.x) a += Wx[x] * rows[(long)k * X + x];
         a = warp_sum(a);
         const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
         if (lane == 0) sm[wid] = a;
@@ -185,19 +197,33 @@ namespace sldg {
 // with fp64 accumulators and the split structure of the rho pass.  The rho and f^2 sums are the very
 // operations, in the very order, of vsum_partial_kernel<.., WITH_S2 = true, ..>, so sldg_diagnostics gives the
 // same bits whichever pass produced its partials.  COMP: compensated rho sum (one-split launches, D:O4).
-template <typename T, int VEC, int DV, int UB, bool COMP>
-__global__ void __launch_bounds__(128)
+template <typename T, int VEC, int DV, int UB, bool COMP, int BLK>
+__global__ void __launch_bounds__(BLK)
 vall_partial_kernel(const T *__restrict__ f, long X, long V, long vps, long part_stride /* cap * X */,
                     const double *__restrict__ Wv, const double *__restrict__ va /* [DV][V] */,
                     const double *__restrict__ v2, double *__restrict__ part) {
     using Vt = Vec<T, VEC>;
+    // The per-row scalars (W_v, |v|^2, v_a) of a chunk of CH rows are staged in shared memory, the next chunk's
+    // prefetched while this one is summed: read through L1 beside the streaming f rows they missed to L2 several
+    // times per batch and every row's arithmetic waited for them (ncu: 33 stall cycles per issue, DRAM at 48 %).
+    constexpr int CH = 64, NT = DV + 2, PER = (NT * CH + BLK - 1) / BLK;   // blockDim.x == BLK
+    __shared__ double s_tab[2][NT][CH];
     const long xv = (long)blockIdx.x * blockDim.x + threadIdx.x;
     const long x = xv * VEC;
-    if (x >= X) return;
+    const bool valid = x < X;
     const long split = blockIdx.y;
     const long v0 = split * vps;
     long v1 = v0 + vps;
     if (v1 > V) v1 = V;
+    auto table_entry = [&](int idx, long c0) -> double {    // entry idx = t * CH + r of the chunk starting at c0
+        const int t = idx / CH, r = idx - t * CH;
+        const long v = c0 + r;
+        if (idx >= NT * CH || v >= v1) return 0.0;
+        return t == 0 ? Wv[v] : (t == 1 ? v2[v] : va[(long)(t - 2) * V + v]);
+    };
+    double pre[PER];
+#pragma unroll
+    for (int i = 0; i < PER; ++i) pre[i] = table_entry((int)threadIdx.x + i * (int)blockDim.x, v0);
     double acc[VEC], lo[VEC], acc2[VEC], mom[DV + 1][VEC];
 #pragma unroll
     for (int e = 0; e < VEC; ++e) {
@@ -205,38 +231,54 @@ vall_partial_kernel(const T *__restrict__ f, long X, long V, long vps, long part
 #pragma unroll
         for (int k = 0; k <= DV; ++k) mom[k][e] = 0.0;
     }
-    const T *p = f + v0 * X + x;
-    auto add_row = [&](const Vt &u, long v) {
-        const double w = Wv[v], s2 = v2[v];
-        double c[DV];
+    const T *p = f + v0 * X + (valid ? x : 0);
+    int cur = 0;
+    for (long c0 = v0; c0 < v1; c0 += CH) {
 #pragma unroll
-        for (int a = 0; a < DV; ++a) c[a] = va[(long)a * V + v];
-#pragma unroll
-        for (int e = 0; e < VEC; ++e) {
-            const double val = (double)u.v[e];
-            const double wv = w * val;
-            if (COMP) comp_add_product(acc[e], lo[e], w, val);
-            else acc[e] += wv;
-            acc2[e] = fma(wv, val, acc2[e]);
-#pragma unroll
-            for (int a = 0; a < DV; ++a) mom[a][e] += c[a] * wv;
-            mom[DV][e] += s2 * wv;
+        for (int i = 0; i < PER; ++i) {
+            const int idx = (int)threadIdx.x + i * (int)blockDim.x;
+            if (idx < NT * CH) (&s_tab[cur][0][0])[idx] = pre[i];
         }
-    };
-    long v = v0;
-    for (; v + UB <= v1; v += UB) {
-        Vt u[UB];
+        __syncthreads();                                     // chunk c0 staged (and the other buffer free again)
 #pragma unroll
-        for (int b = 0; b < UB; ++b) u[b] = *reinterpret_cast<const Vt *>(p + (long)b * X);
+        for (int i = 0; i < PER; ++i) pre[i] = table_entry((int)threadIdx.x + i * (int)blockDim.x, c0 + CH);
+        const int rows = (int)((v1 - c0 < CH) ? v1 - c0 : CH);
+        if (valid) {
+            auto add_row = [&](const Vt &u, int r) {
+                const double w = s_tab[cur][0][r], s2 = s_tab[cur][1][r];
+                double c[DV];
 #pragma unroll
-        for (int b = 0; b < UB; ++b) add_row(u[b], v + b);
-        p += (long)UB * X;
+                for (int a = 0; a < DV; ++a) c[a] = s_tab[cur][2 + a][r];
+#pragma unroll
+                for (int e = 0; e < VEC; ++e) {
+                    const double val = (double)u.v[e];
+                    const double wv = w * val;
+                    if (COMP) comp_add_product(acc[e], lo[e], w, val);
+                    else acc[e] += wv;
+                    acc2[e] = fma(wv, val, acc2[e]);
+#pragma unroll
+                    for (int a = 0; a < DV; ++a) mom[a][e] = fma(c[a], wv, mom[a][e]);
+                    mom[DV][e] = fma(s2, wv, mom[DV][e]);
+                }
+            };
+            int r = 0;
+            for (; r + UB <= rows; r += UB) {
+                Vt u[UB];
+#pragma unroll
+                for (int b = 0; b < UB; ++b) u[b] = *reinterpret_cast<const Vt *>(p + (long)b * X);
+#pragma unroll
+                for (int b = 0; b < UB; ++b) add_row(u[b], r + b);
+                p += (long)UB * X;
+            }
+            for (; r < rows; ++r) {
+                Vt u = *reinterpret_cast<const Vt *>(p);
+                add_row(u, r);
+                p += X;
+            }
+        }
+        cur ^= 1;
     }
-    for (; v < v1; ++v) {
-        Vt u = *reinterpret_cast<const Vt *>(p);
-        add_row(u, v);
-        p += X;
-    }
+    if (!valid) return;
     double *o = part + split * X + x;
 #pragma unroll
     for (int e = 0; e < VEC; ++e) {

@@ -84,6 +84,7 @@ struct sldg_ctx {
     double *d_Wv = nullptr, *d_Wx = nullptr;      // quadrature weights over v-nodes / x-nodes
     double *d_va = nullptr, *d_v2 = nullptr;      // per v-node: coordinates v_a [dv][V] and |v|^2 [V]
     double *d_rho = nullptr, *d_s2 = nullptr, *d_E = nullptr;   // [X], [X], [dx][X]
+    double *d_mom = nullptr;           // [dv + 1][X]: v_a f and |v|^2 f summed over v
     int max_splits = 1;
     double *d_part = nullptr;          // [3 + dv][max_splits][X]: rho, f^2, v_a f, |v|^2 f partials
     double *d_scal = nullptr;          // [8]: mass, l2^2, ee, momentum[dv], |v|^2 moment
@@ -199,7 +200,7 @@ void free_tables(sldg_ctx *c) {
     for (auto &t : c->gen) { cudaFree(t.sigma); cudaFree(t.m); cudaFree(t.ab); }
     for (auto &t : c->xt) { cudaFree(t.sigma); cudaFree(t.m); cudaFree(t.ab); }
     cudaFree(c->d_Wv); cudaFree(c->d_Wx); cudaFree(c->d_va); cudaFree(c->d_v2);
-    cudaFree(c->d_rho); cudaFree(c->d_s2); cudaFree(c->d_E);
+    cudaFree(c->d_rho); cudaFree(c->d_s2); cudaFree(c->d_E); cudaFree(c->d_mom);
     cudaFree(c->d_part); cudaFree(c->d_scal);
     for (int a = 0; a < 3; ++a) { cudaFree(c->d_F[a]); cudaFree(c->d_G[a]); }
     for (int i = 0; i < 4; ++i) cudaFree(c->d_t[i]);
@@ -381,6 +382,7 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
     CREATE_TRY(dalloc(&c->d_rho, c->X));
     CREATE_TRY(dalloc(&c->d_s2, c->X));
     CREATE_TRY(dalloc(&c->d_E, c->X * dx));
+    CREATE_TRY(dalloc(&c->d_mom, c->X * (dv + 1)));
     CREATE_TRY(cudaMemset(c->d_E, 0, c->X * dx * sizeof(double)));
     CREATE_TRY(cudaMemset(c->d_s2, 0, c->X * sizeof(double)));
     CREATE_TRY(dalloc(&c->d_scal, 8));
@@ -1162,12 +1164,11 @@ int run_rho(sldg_ctx *c, double *rho_copy) {
 // a-6 + NEXT-4: ONE read of the current f leaves the partials of rho, f^2, v_a f and |v|^2 f in d_part
 // (vall_partial_kernel) and rho, s2 in d_rho, d_s2; remembered until f changes, so that
 // sldg_diagnostics followed by sldg_moments (or sldg_invariants) reads f once.
-template <typename T, int VEC, int DV, int UB, bool COMP>
-void launch_vall(sldg_ctx *c, int splits, long vps, int block) {
+template <typename T, int VEC, int DV, int UB, bool COMP, int BLK>
+void launch_vall(sldg_ctx *c, int splits, long vps) {
     long xv = c->X / VEC;
-    if (xv < block) block = (int)(cdiv(xv, 32) * 32);
-    dim3 grid((unsigned)cdiv(xv, block), (unsigned)splits);
-    vall_partial_kernel<T, VEC, DV, UB, COMP><<<grid, block, 0, c->stream>>>(
+    dim3 grid((unsigned)cdiv(xv, BLK), (unsigned)splits);
+    vall_partial_kernel<T, VEC, DV, UB, COMP, BLK><<<grid, BLK, 0, c->stream>>>(
         (const T *)c->buf[c->cur], c->X, c->V, vps, (long)c->max_splits * c->X, c->d_Wv, c->d_va, c->d_v2,
         c->d_part);
 }
@@ -1175,17 +1176,22 @@ template <typename T, int DV>
 int run_vall_dv(sldg_ctx *c) {
     constexpr int VMAX = 16 / (int)sizeof(T);
     const VSplit g = vsplit<T>(c);
-    if (g.small) launch_vall<T, 1, DV, 16, true>(c, g.splits, g.vps, 32);
-    else if (g.vec == VMAX) launch_vall<T, VMAX, DV, 4, false>(c, g.splits, g.vps, 128);
-    else if (g.vec == 2) launch_vall<T, 2, DV, 8, false>(c, g.splits, g.vps, 128);
-    else launch_vall<T, 1, DV, 8, false>(c, g.splits, g.vps, 128);
+    if (g.small) launch_vall<T, 1, DV, 16, true, 32>(c, g.splits, g.vps);
+    else if (g.vec == VMAX) launch_vall<T, VMAX, DV, 8, false, 128>(c, g.splits, g.vps);
+    else if (g.vec == 2) launch_vall<T, 2, DV, 8, false, 128>(c, g.splits, g.vps);
+    else launch_vall<T, 1, DV, 8, false, 128>(c, g.splits, g.vps);
     LAUNCH_CHECK(c);
     int rc = finish_vsum(c, g.splits, nullptr, true);
     if (rc) return rc;
     // momentum and |v|^2 moment: sum over splits and x of partials 2 .. 2+dv -> d_scal[3 .. 3+dv]
-    moments_final_kernel<<<1, 1024, 0, c->stream>>>(c->d_part + (size_t)2 * c->max_splits * c->X, c->d_Wx, c->X,
-                                                    g.splits, c->max_splits, c->dv + 1, c->d_scal + 3);
-    LAUNCH_CHECK(c);
+    {
+        const int nk = c->dv + 1, block = 256;
+        vrows_final_kernel<<<(unsigned)cdiv((long)nk * c->X * 32, block), block, 0, c->stream>>>(
+            c->d_part + (size_t)2 * c->max_splits * c->X, c->X, g.splits, c->max_splits, nk, c->d_mom);
+        LAUNCH_CHECK(c);
+        moments_final_kernel<<<1, 1024, 0, c->stream>>>(c->d_mom, c->d_Wx, c->X, nk, c->d_scal + 3);
+        LAUNCH_CHECK(c);
+    }
     c->have_inv = true;
     return SLDG_OK;
 }
