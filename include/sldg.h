@@ -109,7 +109,12 @@ int sldg_advect(sldg_ctx *ctx, int dim, double dt);
  * bit, to sldg_advect(dim1, dt) followed by sldg_advect(dim2, dt) (resp. two sldg_translate_dev
  * calls), but f is read and written once instead of twice.  dim1 < dim2, both x-dimensions or both
  * v-dimensions (their shifts do not depend on each other's coordinate, D:R8).  sldg_step uses this
- * for (x_1,x_2) and (v_1,v_2) unless SLDG_NO_FUSE=1 is set in the environment at sldg_create. */
+ * for (x_1,x_2) and (v_1,v_2) unless SLDG_NO_FUSE=1 is set in the environment at sldg_create.
+ * The fused v-kernels are built for the physical regime |shift| < 1 cell.  sldg_translate_pair_dev /
+ * _triple_dev along v-dimensions therefore assemble the tables first, read back (stream synchronisation)
+ * whether any line is shifted by a cell or more, and run such a call as single sweeps -- same result, two
+ * (three) passes.  sldg_advect_pair / _triple do not check: a field with |E| dt >= h_v is outside the
+ * regime the splitting is accurate in and costs bandwidth there, never correctness. */
 int sldg_advect_pair(sldg_ctx *ctx, int dim1, int dim2, double dt);
 int sldg_translate_pair_dev(sldg_ctx *ctx, int dim1, const double *shift1_device, size_t count1,
                             int dim2, const double *shift2_device, size_t count2);

@@ -88,6 +88,7 @@ struct sldg_ctx {
     int max_splits = 1;
     double *d_part = nullptr;          // [3 + dv][max_splits][X]: rho, f^2, v_a f, |v|^2 f partials
     double *d_scal = nullptr;          // [8]: mass, l2^2, ee, momentum[dv], |v|^2 moment
+    int *d_wide = nullptr;             // [1]: some line of a raw fused v-call is shifted by a cell or more
     // Poisson
     long K[3] = {1, 1, 1}, Mmax[3] = {0, 0, 0}, KK = 1;
     double2 *d_F[3] = {nullptr, nullptr, nullptr}, *d_G[3] = {nullptr, nullptr, nullptr};
@@ -201,7 +202,7 @@ void free_tables(sldg_ctx *c) {
     for (auto &t : c->xt) { cudaFree(t.sigma); cudaFree(t.m); cudaFree(t.ab); }
     cudaFree(c->d_Wv); cudaFree(c->d_Wx); cudaFree(c->d_va); cudaFree(c->d_v2);
     cudaFree(c->d_rho); cudaFree(c->d_s2); cudaFree(c->d_E); cudaFree(c->d_mom);
-    cudaFree(c->d_part); cudaFree(c->d_scal);
+    cudaFree(c->d_part); cudaFree(c->d_scal); cudaFree(c->d_wide);
     for (int a = 0; a < 3; ++a) { cudaFree(c->d_F[a]); cudaFree(c->d_G[a]); }
     for (int i = 0; i < 4; ++i) cudaFree(c->d_t[i]);
     cudaFree(c->d_gh[0]); cudaFree(c->d_gh[1]);
@@ -386,6 +387,7 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
     CREATE_TRY(cudaMemset(c->d_E, 0, c->X * dx * sizeof(double)));
     CREATE_TRY(cudaMemset(c->d_s2, 0, c->X * sizeof(double)));
     CREATE_TRY(dalloc(&c->d_scal, 8));
+    CREATE_TRY(dalloc(&c->d_wide, 1));
     {
         // enough v-splits that X/VEC * splits threads fill the machine (about 2 waves of 2048/SM)
         long target = (long)c->sm_count * 2048 * 2;
@@ -555,13 +557,24 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
             int chunks = (int)cdiv(lpg, R);
             size_t half = ((size_t)R * line_bytes + 127) & ~(size_t)127;
             size_t smem = 2 * half;
-            CUDA_TRY(c, ensure_smem(c, sweep_x1_bulk_kernel<T, O>, smem));
-            long ncell = R * n;
-            int block = ncell >= max_block ? max_block : (int)(cdiv(ncell, 32) * 32);
-            if (block < 64) block = 64;
-            sweep_x1_bulk_kernel<T, O><<<(unsigned)(groups * chunks), block, smem, c->stream>>>(
-                in, out, n, lpg, (int)R, chunks, c->d_m, (const T *)c->d_ab, count, c->N[c->dx], group_stride,
-                line_stride);
+            // O >= 4: a cell's outputs split over two threads
+            constexpr int JH = (O >= 4) ? (O + 1) / 2 : O;
+            auto go = [&](auto kern, int NP) -> int {
+                CUDA_TRY(c, ensure_smem(c, kern, smem));
+                long nitem = R * n * NP;
+                const int mb = max_block;
+                int block = nitem >= mb ? mb : (int)(cdiv(nitem, 32) * 32);
+                if (block < 64) block = 64;
+                if (block % NP) block = (block / NP + 1) * NP;
+                kern<<<(unsigned)(groups * chunks), block, smem, c->stream>>>(
+                    in, out, n, lpg, (int)R, chunks, c->d_m, (const T *)c->d_ab, count, c->N[c->dx], group_stride,
+                    line_stride);
+                return SLDG_OK;
+            };
+            // measured (2+2 D, fp64, GB/s): o = 2 whole cell 6690 / per node 6001; o = 3 whole 6617 / split 5881;
+            // o = 4 whole 5764 / split 7046; o = 6 whole 3700 / split 5663
+            int rc = go(sweep_x1_bulk_kernel<T, O, JH>, (O + JH - 1) / JH);
+            if (rc) return rc;
             done = true;
         }
         if (!done) {
@@ -1074,6 +1087,43 @@ extern "C" int sldg_advect_pair(sldg_ctx *c, int dim1, int dim2, double dt) {
     return commit_tables(c, run_pair(c, dim1, dim2, sweep_count(c, dim1), sweep_count(c, dim2)));
 }
 
+namespace {
+// Raw fused calls along v-dimensions with arbitrary caller shifts: the fused v-kernels are built for the physical
+// regime |shift| < 1 cell (offsets 0 or n-1); with wider shifts neighbouring lanes read cells far apart and the
+// register kernels lose coalescing (measured 70 ms against 2 x 14 ms for a config-4 pair).  The tables are
+// assembled first, with a flag raised by any wider shift; the flag is read back (these raw calls synchronise,
+// like sldg_translate with host shifts) and such a call runs as single TMA sweeps, which do not care.
+int assemble_with_flag(sldg_ctx *c, const int *dims, const size_t *counts, int nd, bool *wide) {
+    CUDA_TRY(c, cudaMemsetAsync(c->d_wide, 0, sizeof(int), c->stream));
+    for (int i = 0; i < nd; ++i) {
+        sldg_ctx::Tab &t = c->gen[i];
+        const int block = 128;
+        const int O = c->o;
+        const size_t sh = (size_t)2 * O * O * 2 * O * 2 * sizeof(double);
+        if (c->dtype == SLDG_F64)
+            assemble_ab_kernel<double><<<(unsigned)cdiv((long)counts[i], block), block, sh, c->stream>>>(
+                t.sigma, (long)counts[i], O, c->cells[dims[i]], c->d_coef, t.m, (double *)t.ab, c->d_wide);
+        else
+            assemble_ab_kernel<float><<<(unsigned)cdiv((long)counts[i], block), block, sh, c->stream>>>(
+                t.sigma, (long)counts[i], O, c->cells[dims[i]], c->d_coef, t.m, (float *)t.ab, c->d_wide);
+        LAUNCH_CHECK(c);
+    }
+    int h = 0;
+    CUDA_TRY(c, cudaMemcpyAsync(&h, c->d_wide, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    *wide = h != 0;
+    return SLDG_OK;
+}
+int singles_from_tables(sldg_ctx *c, const int *dims, const size_t *counts, int nd) {
+    for (int i = 0; i < nd; ++i) {
+        use_tab(c, 1, c->gen[i], true);
+        int rc = run_sweep(c, dims[i], (long)counts[i]);
+        if (rc) return rc;
+    }
+    return SLDG_OK;
+}
+}  // namespace
+
 extern "C" int sldg_translate_pair_dev(sldg_ctx *c, int dim1, const double *shift1, size_t count1, int dim2,
                                        const double *shift2, size_t count2) {
     if (!c || !shift1 || !shift2) return SLDG_ERR_ARG;
@@ -1090,6 +1140,16 @@ extern "C" int sldg_translate_pair_dev(sldg_ctx *c, int dim1, const double *shif
     use_tab(c, 2, c->gen[1], false);
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift1, count1 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma2, shift2, count2 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    if (dim1 >= c->dx) {                 // v-pair: wide shifts run as two single sweeps
+        const int dims[2] = {dim1, dim2};
+        const size_t counts[2] = {count1, count2};
+        bool wide = false;
+        int rc = assemble_with_flag(c, dims, counts, 2, &wide);
+        if (rc) return rc;
+        if (wide) return singles_from_tables(c, dims, counts, 2);
+        use_tab(c, 1, c->gen[0], true);
+        use_tab(c, 2, c->gen[1], true);
+    }
     return run_pair(c, dim1, dim2, (long)count1, (long)count2);
 }
 
@@ -1336,6 +1396,17 @@ extern "C" int sldg_translate_triple_dev(sldg_ctx *c, int dim1, const double *sh
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift1, count1 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma2, shift2, count2 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma3, shift3, count3 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    if (dim1 >= c->dx) {                 // v-triple: wide shifts run as three single sweeps
+        const int dims[3] = {dim1, dim2, dim3};
+        const size_t counts[3] = {count1, count2, count3};
+        bool wide = false;
+        int rc = assemble_with_flag(c, dims, counts, 3, &wide);
+        if (rc) return rc;
+        if (wide) return singles_from_tables(c, dims, counts, 3);
+        use_tab(c, 1, c->gen[0], true);
+        use_tab(c, 2, c->gen[1], true);
+        use_tab(c, 3, c->gen[2], true);
+    }
     return run_triple(c, dim1, dim2, dim3, (long)count1, (long)count2, (long)count3);
 }
 

@@ -35,10 +35,12 @@ __device__ __forceinline__ void dd_horner_step(double &hi, double &lo, double th
     lo = __dadd_rn(se, -__dadd_rn(hi, -s));
 }
 
+// wide (optional): set to 1 when some line's cell offset is neither 0 nor n-1, i.e. |shift| >= 1 cell somewhere
+// (the fused v-kernels keep their loads coalesced only when neighbouring lanes look at neighbouring cells)
 template <typename T>
 __global__ void assemble_ab_kernel(const double *__restrict__ sigma, long count, int o, int n,
                                    const double *__restrict__ coef, int *__restrict__ mtab,
-                                   T *__restrict__ ab) {
+                                   T *__restrict__ ab, int *__restrict__ wide = nullptr) {
     extern __shared__ double s_coef[];             // [2 o^2][2o][hi,lo]
     const int nc = 2 * o, ne = 2 * o * o;
     for (int t = threadIdx.x; t < ne * nc * 2; t += blockDim.x) s_coef[t] = coef[t];
@@ -55,6 +57,7 @@ __global__ void assemble_ab_kernel(const double *__restrict__ sigma, long count,
     int m = (int)mm;
     if (m >= n) m = 0;
     mtab[q] = m;
+    if (wide && m != 0 && m != n - 1) *wide = 1;         // benign race: every writer stores the same value
     for (int e = 0; e < ne; ++e) {
         const double *c = s_coef + (size_t)e * nc * 2;
         double hi = c[(nc - 1) * 2], lo = c[(nc - 1) * 2 + 1];

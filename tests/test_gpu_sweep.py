@@ -155,8 +155,11 @@ def test_tma_and_plain_kernels_agree_bit_for_bit(monkeypatch):
 # ---------------------------------------------------------------- fused pairs (S:8(f) NEXT-1)
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("amp", [3.5, 0.9])
 @pytest.mark.parametrize("o", [1, 2, 3, 4])
-def test_fused_pair_is_bitwise_the_two_sweeps_2p2(oracle, o, dtype):
+def test_fused_pair_is_bitwise_the_two_sweeps_2p2(oracle, o, amp, dtype):
+    """amp = 0.9: |shift| < 1 cell, the regime of the fused v-kernels; amp = 3.5: a raw v-pair with wider
+    shifts is routed to two single sweeps (sldg.h), an x-pair stays one kernel whatever the shift."""
     import torch
     cfg = W.Config("p22", 2, 2, (11, 7, 9, 6), o, (0.0,) * 4, (11.0, 7.0, 9.0, 6.0))
     rng = np.random.default_rng(77 + o)
@@ -165,10 +168,12 @@ def test_fused_pair_is_bitwise_the_two_sweeps_2p2(oracle, o, dtype):
         sig = []
         for k in (k1, k2):
             cnt = cfg.N[cfg.dx + k] if k < cfg.dx else cfg.X
-            sig.append(rng.uniform(-3.5, 3.5, cnt))
+            sig.append(rng.uniform(-amp, amp, cnt))
         a = make_solver(cfg, dtype)
         a.set_initial(f0)
+        l0 = a.launch_count()
         a.translate_pair(k1, torch.from_numpy(sig[0]).cuda(), k2, torch.from_numpy(sig[1]).cuda())
+        assert a.launch_count() - l0 == (4 if (k1 >= 2 and amp > 1.0) else 3)     # 2 table kernels + 1 or 2 sweeps
         fused = a.get_f()
         a.close()
         b = make_solver(cfg, dtype)
@@ -267,15 +272,17 @@ def test_ab_tables_are_rounded_once(oracle, o):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("amp", [2.5, 0.9])
 @pytest.mark.parametrize("o", [1, 2, 3])
-def test_fused_triple_is_bitwise_the_three_sweeps_3p3(oracle, o, dtype):
-    """x_1,x_2,x_3 and v_1,v_2,v_3 in one pass each (o <= 2: the triple kernel; o = 3: pair + single)."""
+def test_fused_triple_is_bitwise_the_three_sweeps_3p3(oracle, o, amp, dtype):
+    """x_1,x_2,x_3 and v_1,v_2,v_3 in one pass each (o <= 2: the triple kernel; o = 3: pair + single);
+    amp = 2.5: the raw v-triple with shifts of a cell or more runs as single sweeps (sldg.h)."""
     import torch
     cfg = W.Config("t33", 3, 3, (5, 4, 6, 4, 5, 3), o, (0.0,) * 6, (5.0, 4.0, 6.0, 4.0, 5.0, 3.0))
     rng = np.random.default_rng(31 + o)
     f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
     for ks in ((0, 1, 2), (3, 4, 5)):
-        sig = [rng.uniform(-2.5, 2.5, cfg.N[cfg.dx + k] if k < cfg.dx else cfg.X) for k in ks]
+        sig = [rng.uniform(-amp, amp, cfg.N[cfg.dx + k] if k < cfg.dx else cfg.X) for k in ks]
         a = make_solver(cfg, dtype)
         a.set_initial(f0)
         a.translate_triple(ks[0], torch.from_numpy(sig[0]).cuda(), ks[1], torch.from_numpy(sig[1]).cuda(),
