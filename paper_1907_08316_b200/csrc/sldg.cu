@@ -53,6 +53,7 @@ struct sldg_ctx {
         int vt_variant = -1;           // SLDG_VTRIPLE_VARIANT: staged v-triple variant (-1 = default)
         bool fuse_rho = true;          // SLDG_NO_FUSE_RHO=1 -> false: rho is a pass of its own after the x-group
         bool rho_triple = false;       // SLDG_RHO_TRIPLE=1: also fuse rho into the x-triple (3+3 D: measured break-even, off)
+        int x1_chunk_kb = 0, x1_block = 128;   // SLDG_X1_CHUNK_KB / SLDG_X1_BLOCK: bulk x_1 kernel geometry (0 = default)
         int rho_cells = 0;             // SLDG_RHO_CELLS: cells per block range in the fused x-group + rho kernels (0 = default)
     } tune;
     // TMA descriptors depend only on (buffer, view), both fixed for the life of the context: encoded once
@@ -280,6 +281,8 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         c->tune.fuse_rho = !env_flag("SLDG_NO_FUSE_RHO");
         c->tune.rho_triple = env_flag("SLDG_RHO_TRIPLE");
         c->tune.rho_cells = env_int("SLDG_RHO_CELLS", 0, 1, 8);
+        c->tune.x1_chunk_kb = env_int("SLDG_X1_CHUNK_KB", 0, 2, 96);
+        c->tune.x1_block = env_int("SLDG_X1_BLOCK", 128, 64, 256) / 32 * 32;
         // columns per tile: a power of two in [8, 128] whose row is a multiple of 16 bytes; anything else is ignored
         int w = env_int("SLDG_TILE_W", 0, 8, 128);
         if (w > 0 && (w & (w - 1)) == 0 && (w * (int)c->esize) % 16 == 0) c->tune.tile_w = w;
@@ -540,10 +543,12 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
         bool done = false;
         if (c->use_tma && line_bytes % 16 == 0 && line_bytes <= 96 * 1024) {
             // staged variant: R whole lines per block through shared memory (bulk copies)
-            // chunk per block: 32 KB (o <= 3) / 16 KB with 128-thread blocks (o >= 4: the per-cell
-            // arithmetic needs ~95+ registers, and only more, smaller blocks keep enough copies in flight)
-            const long chunk_bytes = (O <= 3) ? 32 * 1024 : 16 * 1024;
-            const int max_block = (O <= 3) ? 256 : 128;
+            // 16 KB chunks and 128-thread blocks at every order: ~7 blocks per SM, so that loads, arithmetic and stores
+            // of different blocks overlap (config 4 dim 0, GB/s: 32 KB x 256 threads 6391, 16 KB x 128 7038, 8 KB x 128
+            // 6068, 12 KB x 128 7054, 48 KB x 256 5995; fp32 6198 -> 7045)
+            long chunk_bytes = 16 * 1024;
+            int max_block = 128;
+            if (c->tune.x1_chunk_kb) { chunk_bytes = (long)c->tune.x1_chunk_kb * 1024; max_block = c->tune.x1_block; }
             // shift groups: d_x >= 2: qdiv contiguous lines per (v_1 node, rest); d_x = 1: the lines of one
             // v_1 node are N_v1 lines apart (group = v_1 node, outer / N_v1 strided lines)
             const bool strided_group = (qdiv == 1 && outer > c->N[c->dx]);
