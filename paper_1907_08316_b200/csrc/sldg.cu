@@ -392,11 +392,13 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
     CREATE_TRY(dalloc(&c->d_scal, 8));
     CREATE_TRY(dalloc(&c->d_wide, 1));
     {
-        // enough v-splits that X/VEC * splits threads fill the machine (about 2 waves of 2048/SM)
-        long target = (long)c->sm_count * 2048 * 2;
-        long per = c->X / 2 > 0 ? c->X / 2 : 1;
+        // enough v-splits that X/VEC * splits threads fill the machine several times over (6 waves of 2048/SM: with
+        // 1-2 waves the last, partly filled wave cost up to half the pass -- fp32 config 5 had 1.003 waves, 4.6 TB/s)
+        long target = (long)c->sm_count * 2048 * 6;
+        const long vmax = 16 / (long)c->esize;
+        long per = c->X / vmax > 0 ? c->X / vmax : 1;
         long s = cdiv(target, per);
-        long smax = c->V / 16 > 0 ? c->V / 16 : 1;
+        long smax = c->V / 256 > 0 ? c->V / 256 : 1;     // partials stay under 1/256 of f per quantity
         if (s > smax) s = smax;
         if (s < 1) s = 1;
         if (s > 8192) s = 8192;
@@ -1168,11 +1170,11 @@ int run_poisson_fwd(sldg_ctx *c);
 // v-split geometry shared by the rho pass and the one-read invariants pass
 struct VSplit { int vec; long vps; int splits; bool small; };
 template <typename T>
-VSplit vsplit(const sldg_ctx *c) {
+VSplit vsplit(const sldg_ctx *c, int blocks_per_sm) {
     constexpr int VMAX = 16 / (int)sizeof(T);
     VSplit g;
     g.vec = (c->X % VMAX == 0) ? VMAX : ((c->X % 2 == 0) ? 2 : 1);
-    long target = (long)c->sm_count * 2048 * 2;
+    long target = (long)c->sm_count * 2048 * 6;
     long s = cdiv(target, c->X / g.vec > 0 ? c->X / g.vec : 1);
     if (s > c->max_splits) s = c->max_splits;
     if (s < 1) s = 1;
@@ -1183,6 +1185,12 @@ VSplit vsplit(const sldg_ctx *c) {
     // are short sums and the pass over the splits is compensated.
     g.small = c->V * c->X <= (1L << 23);
     if (g.small) { s = 1; g.vec = 1; }
+    else {
+        // whole waves only: blocks = (blocks along x) * splits just under a multiple of the resident-block count
+        const long bx = cdiv(c->X / g.vec, 128), slots = (long)c->sm_count * blocks_per_sm;
+        const long k = bx * s / slots;
+        if (k >= 1 && k * slots / bx >= 1) s = k * slots / bx;
+    }
     g.vps = cdiv(c->V, s);
     g.splits = (int)cdiv(c->V, g.vps);
     return g;
@@ -1212,7 +1220,7 @@ int finish_vsum(sldg_ctx *c, int splits, double *rho_copy, bool with_s2) {
 template <typename T>
 int run_vsum(sldg_ctx *c, double *rho_copy) {
     constexpr int VMAX = 16 / (int)sizeof(T);
-    const VSplit g = vsplit<T>(c);
+    const VSplit g = vsplit<T>(c, 16);
     c->have_inv = false;                                   // d_part is overwritten
     if (g.small) launch_vsum<T, 1, 32, true>(c, g.splits, g.vps, 32);     // thread per x, 32 rows in flight
     else if (g.vec == VMAX) launch_vsum<T, VMAX, 8>(c, g.splits, g.vps, 128);
@@ -1240,7 +1248,7 @@ void launch_vall(sldg_ctx *c, int splits, long vps) {
 template <typename T, int DV>
 int run_vall_dv(sldg_ctx *c) {
     constexpr int VMAX = 16 / (int)sizeof(T);
-    const VSplit g = vsplit<T>(c);
+    const VSplit g = vsplit<T>(c, 8);
     if (g.small) launch_vall<T, 1, DV, 16, true, 32>(c, g.splits, g.vps);
     else if (g.vec == VMAX) launch_vall<T, VMAX, DV, 8, false, 128>(c, g.splits, g.vps);
     else if (g.vec == 2) launch_vall<T, 2, DV, 8, false, 128>(c, g.splits, g.vps);
