@@ -150,6 +150,19 @@ int sldg_advect_x_rho(sldg_ctx *ctx, double tau, double *rho_device_or_null);
  * x_1..x_dx with dt/2. */
 int sldg_step(sldg_ctx *ctx, double dt);
 
+/* nsteps Strang steps, bit for bit the result of nsteps calls of sldg_step (up to the rounding-level difference
+ * between rho accumulated inside a sweep and rho from its own pass, see sldg_advect_x_rho), with the x
+ * half-steps that end one step and begin the next -- nothing happens between them when no invariant is written
+ * -- done as ONE pass over f: x(dt/2) applied twice inside the kernel (sldg_advect_x_twice), not x(dt).
+ * Per step: v-group (1R+1W), x-group twice (1R+1W), rho (1R) instead of the 7 N s of sldg_step in d_x >= 2.
+ * f(t_n) is materialised only at the end; call sldg_diagnostics etc. between calls of sldg_step_n. */
+int sldg_step_n(sldg_ctx *ctx, double dt, int nsteps);
+
+/* The x-group x_1..x_dx with increment tau applied twice; bit-identical to issuing the group twice.  One pass
+ * over f when one kernel performs the whole group (d_x = 1; d_x = 2 with order <= 3; d_x = 3 with order <= 2
+ * and a small x-grid), else two. */
+int sldg_advect_x_twice(sldg_ctx *ctx, double tau);
+
 /* mass = sum W f, l2 = sqrt(sum W f^2), electric_energy = 1/2 sum_x W_x |E|^2 from the
  * current f (D:R12); recomputes rho and E (they describe the current f afterwards); synchronises the
  * stream.  Any of the three output pointers (host) may be NULL. */

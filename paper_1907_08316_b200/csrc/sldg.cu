@@ -51,6 +51,8 @@ struct sldg_ctx {
         int tile_pair = -1;            // SLDG_TILE_PAIR: -1 default (o >= 3), 0 never, 1 always
         bool tile_triple = true;       // SLDG_NO_TILE_TRIPLE=1 -> false
         int vt_variant = -1;           // SLDG_VTRIPLE_VARIANT: staged v-triple variant (-1 = default)
+        int xt_parts = 0;              // SLDG_XTRIPLE_PARTS: x_2-ranges per velocity node in the x-triple (0 = default, 1 = whole plane)
+        bool twice = true;             // SLDG_NO_TWICE=1 -> false: sldg_step_n never merges the x half-steps of two steps
         bool fuse_rho = true;          // SLDG_NO_FUSE_RHO=1 -> false: rho is a pass of its own after the x-group
         bool rho_triple = false;       // SLDG_RHO_TRIPLE=1: also fuse rho into the x-triple (3+3 D: measured break-even, off)
         int x1_chunk_kb = 0, x1_block = 128;   // SLDG_X1_CHUNK_KB / SLDG_X1_BLOCK: bulk x_1 kernel geometry (0 = default)
@@ -115,6 +117,8 @@ struct sldg_ctx {
     bool use_fuse = true;              // SLDG_NO_FUSE=1: sldg_step issues one sweep per pass
     bool use_tma = true;               // SLDG_NO_TMA=1 in the environment selects the plain kernels
     bool have_rho = false, have_E = false;
+    bool twice_req = false;            // the next x-group kernel should apply the group twice in its one pass
+    bool twice_done = false;           // ... and it did
     bool want_rho = false;             // the next fused x-group sweep should also leave the rho partials (NEXT-1)
     int rho_rows = 0;                  // > 0: that sweep left rho_rows partial rows [rho_rows][X] in d_part
     bool have_inv = false;             // d_part holds the one-read invariant partials of the CURRENT f
@@ -279,6 +283,8 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         c->tune.tile_pair = env_int("SLDG_TILE_PAIR", -1, 0, 1);
         c->tune.vt_variant = env_int("SLDG_VTRIPLE_VARIANT", -1, 0, 15);
         c->tune.fuse_rho = !env_flag("SLDG_NO_FUSE_RHO");
+        c->tune.twice = !env_flag("SLDG_NO_TWICE");
+        c->tune.xt_parts = env_int("SLDG_XTRIPLE_PARTS", 0, 1, 8);
         c->tune.rho_triple = env_flag("SLDG_RHO_TRIPLE");
         c->tune.rho_cells = env_int("SLDG_RHO_CELLS", 0, 1, 8);
         c->tune.x1_chunk_kb = env_int("SLDG_X1_CHUNK_KB", 0, 2, 96);
@@ -580,7 +586,13 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
             };
             // measured (2+2 D, fp64, GB/s): o = 2 whole cell 6690 / per node 6001; o = 3 whole 6617 / split 5881;
             // o = 4 whole 5764 / split 7046; o = 6 whole 3700 / split 5663
-            int rc = go(sweep_x1_bulk_kernel<T, O, JH>, (O + JH - 1) / JH);
+            int rc;
+            if (c->twice_req && c->dx == 1) {            // x(tau) x(tau) of two consecutive steps in one pass
+                rc = go(sweep_x1_bulk_kernel<T, O, JH, true>, (O + JH - 1) / JH);
+                c->twice_done = true;
+            } else {
+                rc = go(sweep_x1_bulk_kernel<T, O, JH>, (O + JH - 1) / JH);
+            }
             if (rc) return rc;
             done = true;
         }
@@ -762,11 +774,23 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
         const long planes = midN * outer2;           // midN == 1 for (0, 1)
         if (c->use_tma && c->tune.plane_pair && k1 == 0 && k2 == 1 && slab_bytes % 16 == 0 && 4 * slot <= 96 * 1024 &&
             n1 <= 256 && n2 >= 3 && planes < (1L << 31)) {
-            CUDA_TRY(c, ensure_smem(c, sweep_xpair_plane_kernel<T, O>, 4 * slot));
             int blk = (int)(cdiv(n1, 32) * 32);
-            sweep_xpair_plane_kernel<T, O><<<(unsigned)planes, blk, 4 * slot, c->stream>>>(
-                in, out, n1, n2, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2, (const T *)c->d_ab2, count2,
-                qd2, qm2);
+            bool twice = false;
+            if constexpr (O <= 3) twice = c->twice_req && c->dx == 2;
+            if (twice) {
+                if constexpr (O <= 3) {                      // x(tau) x(tau) of two consecutive steps in one pass
+                    CUDA_TRY(c, ensure_smem(c, sweep_xpair_plane2_kernel<T, O>, 5 * slot));
+                    sweep_xpair_plane2_kernel<T, O><<<(unsigned)planes, blk, 5 * slot, c->stream>>>(
+                        in, out, n1, n2, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2, (const T *)c->d_ab2,
+                        count2, qd2, qm2);
+                    c->twice_done = true;
+                }
+            } else {
+                CUDA_TRY(c, ensure_smem(c, sweep_xpair_plane_kernel<T, O>, 4 * slot));
+                sweep_xpair_plane_kernel<T, O><<<(unsigned)planes, blk, 4 * slot, c->stream>>>(
+                    in, out, n1, n2, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2, (const T *)c->d_ab2,
+                    count2, qd2, qm2);
+            }
             LAUNCH_CHECK(c);
             c->cur ^= 1;
             f_changed(c);
@@ -908,11 +932,70 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
         const size_t slot = (slab_bytes + 127) & ~(size_t)127;
         if (c->use_tma && k1 == 0 && k2 == 1 && k3 == 2 && c->dx == 3 && slab_bytes % 16 == 0 &&
             4 * slot <= 200 * 1024 && (long)n1 * n2 <= 512 && outer3 < (1L << 31)) {
-            CUDA_TRY(c, ensure_smem(c, sweep_xtriple_plane_kernel<T, O>, 4 * slot));
-            int block = (int)(cdiv((long)n1 * n2, 32) * 32);
-            sweep_xtriple_plane_kernel<T, O><<<(unsigned)outer3, block, 4 * slot, c->stream>>>(
-                in, out, n1, n2, n3, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2,
-                qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+            // Part-plane blocks (nb2 ranges of x_2-cells per velocity node): two resident blocks whose phases overlap
+            {
+                // (config 5: single application 12.2 -> 11.5 ms; applied twice the part kernel spills and computes a row
+                //  of cells redundantly: 22.9 ms against 21.1 ms for the whole plane, so twice stays on whole planes
+                //  unless SLDG_XTRIPLE_PARTS asks otherwise)
+                const int nb2 = c->tune.xt_parts ? c->tune.xt_parts : (c->twice_req ? 1 : 2);
+                const int apps = c->twice_req ? 2 : 1;
+                if (nb2 >= 2 && n2 % nb2 == 0 && n2 / nb2 >= 2) {
+                    const int c2b = n2 / nb2;
+                    const long thr = (long)(c2b + apps - 1) * n1;
+                    const int blk = (int)(cdiv(thr, 32) * 32);
+                    const size_t rowb = (size_t)O * n1 * sizeof(T);          // one row of the (x_1,x_2)-plane
+                    const size_t slot_p = ((size_t)O * (c2b + apps) * O * rowb + 127) & ~(size_t)127;
+                    const size_t tb_p = ((size_t)O * (c2b + apps - 1) * O * rowb + 127) & ~(size_t)127;
+                    const size_t smem_p = (apps == 1 ? 4 * slot_p : 3 * slot_p + 2 * tb_p) +
+                                          (size_t)apps * O * O * O * blk * sizeof(T);
+                    if (thr <= 256 && smem_p <= 110 * 1024 && rowb % 16 == 0 && outer3 * nb2 < (1L << 31)) {
+                        cudaError_t e;
+                        if (apps == 2) {
+                            auto kern = sweep_xtriple_part_kernel<T, O, 2>;
+                            e = ensure_smem(c, kern, smem_p);
+                            if (e == cudaSuccess)
+                                kern<<<(unsigned)(outer3 * nb2), blk, smem_p, c->stream>>>(
+                                    in, out, n1, n2, n3, c2b, nb2, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1],
+                                    (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+                        } else {
+                            auto kern = sweep_xtriple_part_kernel<T, O, 1>;
+                            e = ensure_smem(c, kern, smem_p);
+                            if (e == cudaSuccess)
+                                kern<<<(unsigned)(outer3 * nb2), blk, smem_p, c->stream>>>(
+                                    in, out, n1, n2, n3, c2b, nb2, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1],
+                                    (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+                        }
+                        if (e == cudaSuccess) {
+                            LAUNCH_CHECK(c);
+                            if (apps == 2) c->twice_done = true;
+                            c->cur ^= 1;
+                            f_changed(c);
+                            return SLDG_OK;
+                        }
+                        cudaGetLastError();
+                    }
+                }
+            }
+            // threads per x_2-cell row: dense.  (n1 rounded up to a multiple of 8 makes the 16-byte shared-memory
+            // accesses conflict-free -- with n1 = 20 a quarter warp straddles two rows, 23 % of the wavefronts are
+            // conflicts -- but the idle lanes cost more: config 5 triple 11.7 -> 12.2 ms, applied twice 20.7 -> 24.6 ms)
+            int tpr = n1;
+            int block = (int)(cdiv((long)tpr * n2, 32) * 32);
+            // twice: ring + the first application's cell + the two parked first cells of the windows
+            const size_t smem2 = 5 * slot + (size_t)2 * O * O * O * block * sizeof(T);   // 3-deep ring, 2 cells, parked
+            if (c->twice_req && smem2 <= 226 * 1024 &&
+                ensure_smem(c, sweep_xtriple_plane2_kernel<T, O>, smem2) == cudaSuccess) {
+                sweep_xtriple_plane2_kernel<T, O><<<(unsigned)outer3, block, smem2, c->stream>>>(
+                    in, out, n1, n2, n3, tpr, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2,
+                    qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+                c->twice_done = true;
+            } else {
+                cudaGetLastError();
+                CUDA_TRY(c, ensure_smem(c, sweep_xtriple_plane_kernel<T, O>, 4 * slot));
+                sweep_xtriple_plane_kernel<T, O><<<(unsigned)outer3, block, 4 * slot, c->stream>>>(
+                    in, out, n1, n2, n3, tpr, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2,
+                    qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+            }
             LAUNCH_CHECK(c);
             c->cur ^= 1;
             f_changed(c);
@@ -1426,12 +1509,15 @@ extern "C" int sldg_translate_triple_dev(sldg_ctx *c, int dim1, const double *sh
 namespace {
 // sweeps along dimensions base .. base+cnt-1 with increment tau, fusing the first two when allowed;
 // with_rho: the fused kernel that performs the WHOLE group may also leave the rho partials (c->rho_rows)
-int advect_group(sldg_ctx *c, int base, int cnt, double tau, bool with_rho = false) {
+int advect_group(sldg_ctx *c, int base, int cnt, double tau, bool with_rho = false, bool twice = false) {
     int rc, a = 0;
     c->rho_rows = 0;
     const bool whole = c->use_fuse && ((cnt == 3 && c->o <= 2) || (cnt == 2 && c->o <= 4));
     c->want_rho = with_rho && whole && c->tune.fuse_rho && base == 0;
-    struct Clear { sldg_ctx *c; ~Clear() { c->want_rho = false; } } clear{c};
+    // twice: only a kernel that performs the WHOLE group may apply it twice in its pass (c->twice_done tells)
+    c->twice_req = twice && base == 0 && c->tune.twice && (whole || cnt == 1);
+    c->twice_done = false;
+    struct Clear { sldg_ctx *c; ~Clear() { c->want_rho = false; c->twice_req = false; } } clear{c};
     if (c->use_fuse && cnt == 3 && c->o <= 2) return sldg_advect_triple(c, base, base + 1, base + 2, tau);
     if (c->use_fuse && cnt >= 2) {
         if ((rc = sldg_advect_pair(c, base, base + 1, tau))) return rc;
@@ -1453,6 +1539,15 @@ int advect_x_rho(sldg_ctx *c, double tau, double *rho_copy) {
         return finish_vsum(c, rows, rho_copy, false);
     }
     return run_rho(c, rho_copy);
+}
+
+// the x-group applied twice with increment tau: one pass when a kernel takes the whole group (plane kernels,
+// bulk x_1 kernel), else the group twice; bit-identical either way
+int advect_x_twice(sldg_ctx *c, double tau) {
+    int rc = advect_group(c, 0, c->dx, tau, false, true);
+    if (rc) return rc;
+    if (c->twice_done) { c->twice_done = false; return SLDG_OK; }
+    return advect_group(c, 0, c->dx, tau);
 }
 
 int step_body(sldg_ctx *c, double dt) {
@@ -1498,6 +1593,40 @@ int capture_step(sldg_ctx *c, double dt, sldg_ctx::StepGraph &g) {
     return SLDG_OK;
 }
 }  // namespace
+
+extern "C" int sldg_advect_x_twice(sldg_ctx *c, double tau) {
+    if (!c) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
+    return advect_x_twice(c, tau);
+}
+
+extern "C" int sldg_step_n(sldg_ctx *c, double dt, int nsteps) {
+    if (!c || nsteps < 0) return SLDG_ERR_ARG;
+    if (nsteps == 0) return SLDG_OK;
+    // launch-bound problems replay the CUDA graph of one step; merging is for the bandwidth-bound ones
+    if (c->use_graph || nsteps == 1 || !c->tune.twice) {
+        for (int s = 0; s < nsteps; ++s) {
+            int rc = sldg_step(c, dt);
+            if (rc) return rc;
+        }
+        return SLDG_OK;
+    }
+    DeviceGuard guard(c);
+    int rc;
+    if ((rc = advect_x_rho(c, 0.5 * dt, nullptr))) return rc;
+    for (int s = 0; s < nsteps; ++s) {
+        if ((rc = run_poisson(c, nullptr))) return rc;
+        if ((rc = advect_group(c, c->dx, c->dx, dt))) return rc;
+        if (s + 1 < nsteps) {
+            // the last x half-step of this step and the first of the next: x(dt/2) x(dt/2) in one pass, then rho
+            if ((rc = advect_x_twice(c, 0.5 * dt))) return rc;
+            if ((rc = run_rho(c, nullptr))) return rc;
+        } else {
+            if ((rc = advect_group(c, 0, c->dx, 0.5 * dt))) return rc;
+        }
+    }
+    return SLDG_OK;
+}
 
 extern "C" int sldg_advect_x_rho(sldg_ctx *c, double tau, double *rho_out) {
     if (!c) return SLDG_ERR_ARG;

@@ -364,7 +364,7 @@ namespace sldg {
 // ------------------------------------------------------------------------------------------
 template <typename T, int O>
 __global__ void __launch_bounds__(512, 1)
-sweep_xtriple_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2, int n3,
+sweep_xtriple_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2, int n3, int tpr,
                            const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
                            const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2,
                            const int *__restrict__ mtab3, const T *__restrict__ ab3, long count3, long qdiv3, long qmod3) {
@@ -378,8 +378,10 @@ sweep_xtriple_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1
     const long v = blockIdx.x;
     const long base = v * (long)n3 * slab;                   // first element of this v (x-block is contiguous)
     const int tid = threadIdx.x;
-    const int c1 = tid % n1, c2 = tid / n1;
-    const bool active = c2 < n2;
+    // tpr threads per x_2-cell row, n1 of them active (tpr > n1 pads rows for bank conflicts; measured slower)
+    const int c1r = tid % tpr, c2 = tid / tpr;
+    const bool active = c2 < n2 && c1r < n1;
+    const int c1 = c1r < n1 ? c1r : 0;
 
     const long q1 = (base / qdiv1) % qmod1, q2 = (base / qdiv2) % qmod2, q3 = (base / qdiv3) % qmod3;
     T A1[O * O], B1[O * O], A2[O * O], B2[O * O], A3[O * O], B3[O * O];
@@ -1415,6 +1417,621 @@ sweep_xtriple_rho_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, 
     __syncthreads();
     double *pr = part + chunk * (long)n3 * slab + (long)i0 * slab;     // row `chunk` of [nchunk][X], X = n3 * slab
     for (long e = tid; e < (long)ncell * slab; e += blockDim.x) pr[e] = racc[e];
+}
+
+}  // namespace sldg
+
+namespace sldg {
+
+// ------------------------------------------------------------------------------------------
+// The x-group applied TWICE in one pass over f.  Consecutive Strang steps end and begin with the same
+// x half-step, and nothing separates the two when no invariant is written in between: x(tau) x(tau) is
+// then one read and one write of f instead of two of each.  NOT x(2 tau): each application is the full O7 chain
+// of the single sweeps, so the result is bit-identical to calling the x-group twice (sldg_step_n relies on it).
+//
+// x_1 x_2 pair, one block per (x_1,x_2) plane as sweep_xpair_plane_kernel: the first application's output cell
+// (O x O values per thread) goes to a slab-sized shared-memory buffer instead of global memory; after a barrier
+// every thread reads its two x_1 source cells of it and runs the second application with a second window.  The
+// shifts, A and B are those of the first application (same tau, same v).  Output cells leave in the order the
+// second window closes them: cell (i - 1 - m2) mod n2 when the first application has produced its cell i.
+// ------------------------------------------------------------------------------------------
+template <typename T, int O>
+__global__ void __launch_bounds__(256)
+sweep_xpair_plane2_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2,
+                          const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
+                          const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    constexpr int NS = 4;                                   // ring depth
+    __shared__ __align__(8) uint64_t full[NS];
+    const long N1 = (long)n1 * O;
+    const long slab = O * N1;                                // elements per k2-cell of one plane
+    const size_t slab_bytes = (size_t)slab * sizeof(T);
+    const size_t slot_stride = (slab_bytes + 127) & ~(size_t)127;
+    T *tbuf = reinterpret_cast<T *>(smem_raw + NS * slot_stride);   // the first application's current output cell
+    const long base = (long)blockIdx.x * n2 * slab;          // planes are contiguous
+    const int tid = threadIdx.x;
+    const int c1 = tid;
+    const bool active = c1 < n1;
+
+    const long q1 = (base / qdiv1) % qmod1, q2 = (base / qdiv2) % qmod2;
+    T A1[O * O], B1[O * O], A2[O * O], B2[O * O];
+#pragma unroll
+    for (int e = 0; e < O * O; ++e) {
+        A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1];
+        A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
+    }
+    const int m1 = mtab1[q1], m2 = mtab2[q2];
+    int sa1 = (active ? c1 : 0) + m1; if (sa1 >= n1) sa1 -= n1;
+    int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+    }
+    __syncthreads();
+    auto issue = [&](int j) {                                // slab j <-> source k2-cell (m2 + j) mod n2
+        int cell = m2 + j;
+        if (cell >= n2) cell -= n2;
+        const int slot = j % NS;
+        mbar_expect_tx(&full[slot], (uint32_t)slab_bytes);
+        bulk_g2s(smem_raw + slot * slot_stride, in + base + (long)cell * slab, (uint32_t)slab_bytes, &full[slot]);
+    };
+    if (tid == 0)
+        for (int j = 0; j < NS && j < n2; ++j) issue(j);
+
+    auto k1_from = [&](const T *sl, T (&w)[O][O]) {          // w[l2][j1]: k1 rule on this thread's two source cells
+#pragma unroll
+        for (int l2 = 0; l2 < O; ++l2) {
+            T r0[O], r1[O];
+            load_cell<T, O>(sl + l2 * N1 + (long)sa1 * O, r0);
+            load_cell<T, O>(sl + l2 * N1 + (long)sb1 * O, r1);
+#pragma unroll
+            for (int j1 = 0; j1 < O; ++j1) w[l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+        }
+    };
+    auto a_half = [&](const T (&w)[O][O], T (&acc)[O][O]) {  // k2 rule, A row on the older cell
+#pragma unroll
+        for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+            for (int j1 = 0; j1 < O; ++j1) {
+                T a = mul_t<T>(A2[j2 * O], w[0][j1]);
+#pragma unroll
+                for (int l = 1; l < O; ++l) a = fma_t<T>(A2[j2 * O + l], w[l][j1], a);
+                acc[j2][j1] = a;
+            }
+    };
+    auto b_half = [&](const T (&acc)[O][O], const T (&w)[O][O], T (&res)[O][O]) {   // ... B row on the newer one
+#pragma unroll
+        for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+            for (int j1 = 0; j1 < O; ++j1) {
+                T a = acc[j2][j1];
+#pragma unroll
+                for (int l = 0; l < O; ++l) a = fma_t<T>(B2[j2 * O + l], w[l][j1], a);
+                res[j2][j1] = a;
+            }
+    };
+    auto put = [&](T *dst_cell, long row_stride, const T (&res)[O][O]) {           // O rows of O values
+#pragma unroll
+        for (int j2 = 0; j2 < O; ++j2) {
+            T *p = dst_cell + (long)j2 * row_stride;
+            if constexpr (O % 2 == 0) {
+                using V2 = Vec<T, 2>;
+#pragma unroll
+                for (int j1 = 0; j1 < O; j1 += 2) {
+                    V2 vv; vv.v[0] = res[j2][j1]; vv.v[1] = res[j2][j1 + 1];
+                    *reinterpret_cast<V2 *>(p + j1) = vv;
+                }
+            } else {
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) p[j1] = res[j2][j1];
+            }
+        }
+    };
+
+    T wfirst[O][O], acc1[O][O], bfirst[O][O], acc2[O][O];
+    // second application on the first one's output cell i (in tbuf, visible to all threads)
+    auto second = [&](int i) {
+        if (!active) return;
+        T b[O][O];
+        k1_from(tbuf, b);
+        if (i == 0) {
+#pragma unroll
+            for (int a = 0; a < O; ++a)
+#pragma unroll
+                for (int d = 0; d < O; ++d) bfirst[a][d] = b[a][d];
+        } else {
+            T res[O][O];
+            b_half(acc2, b, res);
+            int cell = i - 1 - m2;
+            if (cell < 0) cell += n2;
+            put(out + base + (long)cell * slab + (long)c1 * O, N1, res);
+        }
+        a_half(b, acc2);
+    };
+
+    for (int j = 0; j < n2; ++j) {
+        const int slot = j % NS;
+        mbar_wait(&full[slot], (uint32_t)((j / NS) & 1));
+        T w[O][O];
+        if (active) k1_from(reinterpret_cast<const T *>(smem_raw + slot * slot_stride), w);
+        __syncthreads();                                     // slab consumed (and tbuf no longer read)
+        if (tid == 0 && j + NS < n2) issue(j + NS);
+        if (j == 0) {
+            if (active) {
+#pragma unroll
+                for (int a = 0; a < O; ++a)
+#pragma unroll
+                    for (int d = 0; d < O; ++d) wfirst[a][d] = w[a][d];
+                a_half(w, acc1);
+            }
+        } else {
+            if (active) {
+                T res[O][O];
+                b_half(acc1, w, res);                        // first application, cell j - 1
+                a_half(w, acc1);
+                put(tbuf + (long)c1 * O, N1, res);
+            }
+            __syncthreads();
+            second(j - 1);
+        }
+    }
+    __syncthreads();                                         // tbuf no longer read
+    if (active) {
+        T res[O][O];
+        b_half(acc1, wfirst, res);                           // first application, cell n2 - 1 (closes the line)
+        put(tbuf + (long)c1 * O, N1, res);
+    }
+    __syncthreads();
+    second(n2 - 1);
+    if (active) {
+        T res[O][O];
+        b_half(acc2, bfirst, res);                           // second application closes its line
+        int cell = n2 - 1 - m2;
+        if (cell < 0) cell += n2;
+        put(out + base + (long)cell * slab + (long)c1 * O, N1, res);
+    }
+}
+
+// x_1 x_2 x_3 triple applied twice, one block per velocity node as sweep_xtriple_plane_kernel.  The two windows'
+// first cells (needed only to close the periodic lines at the very end) are parked in shared memory, so the
+// register budget is that of the single application.
+template <typename T, int O>
+__global__ void __launch_bounds__(512, 1)
+sweep_xtriple_plane2_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2, int n3, int tpr,
+                            const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
+                            const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2,
+                            const int *__restrict__ mtab3, const T *__restrict__ ab3, long count3, long qdiv3, long qmod3) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    constexpr int NS = 3;
+    constexpr int O3 = O * O * O;
+    __shared__ __align__(8) uint64_t full[NS], tbar[2];
+    const long N1 = (long)n1 * O, N2 = (long)n2 * O;
+    const long slab = O * N2 * N1;                           // elements per k3-cell
+    const size_t slab_bytes = (size_t)slab * sizeof(T);
+    const size_t slot_stride = (slab_bytes + 127) & ~(size_t)127;
+    // the first application's output cells, double-buffered: cell i is written during iteration i + 1 and read
+    // during iteration i + 2, so the barrier between the two (an mbarrier counted in threads: arrive after the
+    // write, wait before the read) has a whole iteration to complete and nobody stalls at it
+    T *tbuf0 = reinterpret_cast<T *>(smem_raw + NS * slot_stride);
+    T *park = reinterpret_cast<T *>(smem_raw + (NS + 2) * slot_stride);   // [2][O3][blockDim]
+    const long v = blockIdx.x;
+    const long base = v * (long)n3 * slab;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int c1r = tid % tpr, c2 = tid / tpr;               // tpr threads per row, n1 active (bank conflicts, see above)
+    const bool active = c2 < n2 && c1r < n1;
+    const int c1 = c1r < n1 ? c1r : 0;
+
+    const long q1 = (base / qdiv1) % qmod1, q2 = (base / qdiv2) % qmod2, q3 = (base / qdiv3) % qmod3;
+    T A1[O * O], B1[O * O], A2[O * O], B2[O * O], A3[O * O], B3[O * O];
+#pragma unroll
+    for (int e = 0; e < O * O; ++e) {
+        A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1];
+        A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
+        A3[e] = ab3[(long)e * count3 + q3]; B3[e] = ab3[(long)(O * O + e) * count3 + q3];
+    }
+    const int m1 = mtab1[q1], m2 = mtab2[q2], m3 = mtab3[q3];
+    int sa1 = c1 + m1; if (sa1 >= n1) sa1 -= n1;
+    int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
+    int sa2 = (active ? c2 : 0) + m2; if (sa2 >= n2) sa2 -= n2;
+    int sb2 = sa2 + 1; if (sb2 == n2) sb2 = 0;
+    const int off[2][2] = {{(int)(sa2 * O * N1 + sa1 * O), (int)(sa2 * O * N1 + sb1 * O)},
+                           {(int)(sb2 * O * N1 + sa1 * O), (int)(sb2 * O * N1 + sb1 * O)}};
+    const long cell_off = (long)c2 * O * N1 + (long)c1 * O;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+        mbar_init(&tbar[0], nthr);
+        mbar_init(&tbar[1], nthr);
+    }
+    __syncthreads();
+    auto issue = [&](int j) {                                // slab j <-> source k3-cell (m3 + j) mod n3
+        int cell = m3 + j;
+        if (cell >= n3) cell -= n3;
+        const int slot = j % NS;
+        mbar_expect_tx(&full[slot], (uint32_t)slab_bytes);
+        bulk_g2s(smem_raw + slot * slot_stride, in + base + (long)cell * slab, (uint32_t)slab_bytes, &full[slot]);
+    };
+    if (tid == 0)
+        for (int j = 0; j < NS && j < n3; ++j) issue(j);
+
+    auto k12_from = [&](const T *sl, T (&w)[O][O][O]) {      // (k1,k2)-swept values of this thread's cell pair
+#pragma unroll
+        for (int l3 = 0; l3 < O; ++l3) {
+            T tk[2][O][O];
+#pragma unroll
+            for (int e2 = 0; e2 < 2; ++e2)
+#pragma unroll
+                for (int l2 = 0; l2 < O; ++l2) {
+                    T r0[O], r1[O];
+                    load_cell<T, O>(sl + l3 * N2 * N1 + off[e2][0] + l2 * N1, r0);
+                    load_cell<T, O>(sl + l3 * N2 * N1 + off[e2][1] + l2 * N1, r1);
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) tk[e2][l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+                }
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a0[O], a1[O];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) { a0[l] = tk[0][l][j1]; a1[l] = tk[1][l][j1]; }
+                    w[l3][j2][j1] = chain<T, O>(A2, B2, j2, a0, a1);
+                }
+        }
+    };
+    auto a_half = [&](const T (&w)[O][O][O], T (&acc)[O][O][O]) {
+#pragma unroll
+        for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a = mul_t<T>(A3[j3 * O], w[0][j2][j1]);
+#pragma unroll
+                    for (int l = 1; l < O; ++l) a = fma_t<T>(A3[j3 * O + l], w[l][j2][j1], a);
+                    acc[j3][j2][j1] = a;
+                }
+    };
+    // B-half of the k3 rule and the O^3 results written as O^2 rows of O values at dst (row pitches N1, N2*N1)
+    auto b_half_put = [&](const T (&acc)[O][O][O], const T (&w)[O][O][O], T *dst) {
+#pragma unroll
+        for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2) {
+                T res[O];
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a = acc[j3][j2][j1];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) a = fma_t<T>(B3[j3 * O + l], w[l][j2][j1], a);
+                    res[j1] = a;
+                }
+                T *p = dst + (long)j3 * N2 * N1 + (long)j2 * N1;
+                if constexpr (O % 2 == 0) {
+                    using V2 = Vec<T, 2>;
+#pragma unroll
+                    for (int j1 = 0; j1 < O; j1 += 2) {
+                        V2 vv; vv.v[0] = res[j1]; vv.v[1] = res[j1 + 1];
+                        *reinterpret_cast<V2 *>(p + j1) = vv;
+                    }
+                } else {
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) p[j1] = res[j1];
+                }
+            }
+    };
+    auto park_put = [&](int which, const T (&w)[O][O][O]) {
+#pragma unroll
+        for (int a = 0; a < O; ++a)
+#pragma unroll
+            for (int b = 0; b < O; ++b)
+#pragma unroll
+                for (int d = 0; d < O; ++d) park[((which * O3) + (a * O + b) * O + d) * nthr + tid] = w[a][b][d];
+    };
+    auto park_get = [&](int which, T (&w)[O][O][O]) {
+#pragma unroll
+        for (int a = 0; a < O; ++a)
+#pragma unroll
+            for (int b = 0; b < O; ++b)
+#pragma unroll
+                for (int d = 0; d < O; ++d) w[a][b][d] = park[((which * O3) + (a * O + b) * O + d) * nthr + tid];
+    };
+
+    T acc1[O][O][O], acc2[O][O][O];
+    auto tb = [&](int i) -> T * { return tbuf0 + (size_t)(i & 1) * (slot_stride / sizeof(T)); };
+    auto second = [&](int i) {                               // second application on the first one's cell i
+        mbar_wait(&tbar[i & 1], (uint32_t)((i >> 1) & 1));   // every thread has written its part of cell i
+        if (!active) return;
+        T b[O][O][O];
+        k12_from(tb(i), b);
+        if (i == 0) {
+            park_put(1, b);
+        } else {
+            int cell = i - 1 - m3;
+            if (cell < 0) cell += n3;
+            b_half_put(acc2, b, out + base + (long)cell * slab + cell_off);
+        }
+        a_half(b, acc2);
+    };
+
+    for (int j = 0; j < n3; ++j) {
+        const int slot = j % NS;
+        mbar_wait(&full[slot], (uint32_t)((j / NS) & 1));
+        T w[O][O][O];
+        if (active) k12_from(reinterpret_cast<const T *>(smem_raw + slot * slot_stride), w);
+        __syncthreads();                                     // slab consumed; everybody is through iteration j - 1
+        if (tid == 0 && j + NS < n3) issue(j + NS);
+        if (j == 0) {
+            if (active) { park_put(0, w); a_half(w, acc1); }
+        } else {
+            if (active) {
+                b_half_put(acc1, w, tb(j - 1) + cell_off);   // first application, cell j - 1
+                a_half(w, acc1);
+            }
+            mbar_arrive(&tbar[(j - 1) & 1]);
+            if (j >= 2) second(j - 2);
+        }
+    }
+    __syncthreads();
+    if (active) {
+        T wf[O][O][O];
+        park_get(0, wf);
+        b_half_put(acc1, wf, tb(n3 - 1) + cell_off);         // first application closes its line
+    }
+    mbar_arrive(&tbar[(n3 - 1) & 1]);
+    second(n3 - 2);
+    second(n3 - 1);
+    if (active) {
+        T bf[O][O][O];
+        park_get(1, bf);
+        int cell = n3 - 1 - m3;
+        if (cell < 0) cell += n3;
+        b_half_put(acc2, bf, out + base + (long)cell * slab + cell_off);
+    }
+}
+
+}  // namespace sldg
+
+namespace sldg {
+
+// ------------------------------------------------------------------------------------------
+// x_1 x_2 x_3 triple (APPS = 1) or the triple applied twice (APPS = 2), one block per velocity node AND per
+// RANGE of x_2-cells (nb2 blocks per node).  The whole-plane kernels above keep one block of ~13 warps per SM,
+// all in the same phase (shared-memory loads, then FMA chains, then the barrier): the LSU and the fp64 pipe are
+// each busy about half of the time and their phases add up (ncu, profiles/ncu_twice_r2.md).  Half the plane per
+// block halves threads and shared memory, two blocks are resident and their phases overlap.
+//
+// A block owns the x_2-cells [c2_0, c2_0 + c2b) of one node v.  Its outputs need the source cells
+// c2_0 + APPS m2 ... c2_0 + APPS m2 + c2b + APPS - 1 (periodic): per x_3-cell (slab) and x_3-node one contiguous
+// piece of rows of the (x_1,x_2)-plane, two when it wraps, brought in by cp.async.bulk; the extra cells are the
+// x_2 neighbours (L2 hits for the block next door).  With APPS = 2 the first application is computed for
+// c2b + 1 cells (one redundantly), staged in shared memory, and the second runs on it as in
+// sweep_xtriple_plane2_kernel.  Bit-identical to the single sweeps.
+// ------------------------------------------------------------------------------------------
+template <typename T, int O, int APPS>
+__global__ void __launch_bounds__(256, 2)
+sweep_xtriple_part_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2, int n3, int c2b, int nb2,
+                          const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
+                          const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2,
+                          const int *__restrict__ mtab3, const T *__restrict__ ab3, long count3, long qdiv3, long qmod3) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    constexpr int NS = (APPS == 1) ? 4 : 3;
+    constexpr int O3 = O * O * O;
+    __shared__ __align__(8) uint64_t full[NS], tbar[2];
+    const long N1 = (long)n1 * O, N2 = (long)n2 * O;
+    const long slab = O * N2 * N1;                           // elements per x_3-cell of one node (global)
+    const int RC = c2b + APPS;                               // staged x_2-cells
+    const int nT = c2b + APPS - 1;                           // cells the first application is computed for
+    const long PR = (long)RC * O;                            // staged rows per x_3-node
+    const long lslab = O * PR * N1;                          // elements of a staged slab
+    const size_t slot_stride = ((size_t)lslab * sizeof(T) + 127) & ~(size_t)127;
+    const long TR = (long)nT * O;                            // rows per x_3-node of the first application's cell
+    const size_t tb_stride = ((size_t)O * TR * N1 * sizeof(T) + 127) & ~(size_t)127;
+    T *tbuf0 = reinterpret_cast<T *>(smem_raw + NS * slot_stride);
+    T *park = reinterpret_cast<T *>(smem_raw + NS * slot_stride + (APPS == 2 ? 2 * tb_stride : 0));   // [APPS][O3][blockDim]
+    const long v = blockIdx.x / nb2;
+    const int c2_0 = (int)(blockIdx.x % nb2) * c2b;
+    const long base = v * (long)n3 * slab;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int c1 = tid % n1, t2 = tid / n1;
+    const bool act1 = t2 < nT;                               // computes a cell of the first application
+    const bool act2 = t2 < c2b;                              // computes an output cell
+
+    const long q1 = (base / qdiv1) % qmod1, q2 = (base / qdiv2) % qmod2, q3 = (base / qdiv3) % qmod3;
+    T A1[O * O], B1[O * O], A2[O * O], B2[O * O], A3[O * O], B3[O * O];
+#pragma unroll
+    for (int e = 0; e < O * O; ++e) {
+        A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1];
+        A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
+        A3[e] = ab3[(long)e * count3 + q3]; B3[e] = ab3[(long)(O * O + e) * count3 + q3];
+    }
+    const int m1 = mtab1[q1], m2 = mtab2[q2], m3 = mtab3[q3];
+    int sa1 = c1 + m1; if (sa1 >= n1) sa1 -= n1;
+    int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
+    const int t2c = act1 ? t2 : 0;
+    // offsets of the 2 x 2 source cells in a staged slab / in the first application's cell: local rows t2, t2 + 1
+    const int off[2][2] = {{(int)(t2c * O * N1 + sa1 * O), (int)(t2c * O * N1 + sb1 * O)},
+                           {(int)((t2c + 1) * O * N1 + sa1 * O), (int)((t2c + 1) * O * N1 + sb1 * O)}};
+    int rs = c2_0 + APPS * m2;                               // first staged x_2-cell (global index)
+    rs %= n2;
+    const int first_cells = (rs + RC <= n2) ? RC : n2 - rs;  // cells before the periodic wrap
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+        mbar_init(&tbar[0], nthr);
+        mbar_init(&tbar[1], nthr);
+    }
+    __syncthreads();
+    auto issue = [&](int j) {                                // slab j <-> source x_3-cell (m3 + j) mod n3
+        int cell = m3 + j;
+        if (cell >= n3) cell -= n3;
+        const int slot = j % NS;
+        T *dst = reinterpret_cast<T *>(smem_raw + slot * slot_stride);
+        mbar_expect_tx(&full[slot], (uint32_t)((size_t)lslab * sizeof(T)));
+        const T *src = in + base + (long)cell * slab;
+#pragma unroll
+        for (int l3 = 0; l3 < O; ++l3) {
+            const uint32_t b1 = (uint32_t)((size_t)first_cells * O * N1 * sizeof(T));
+            bulk_g2s(dst + l3 * PR * N1, src + l3 * N2 * N1 + (long)rs * O * N1, b1, &full[slot]);
+            if (first_cells < RC)
+                bulk_g2s(dst + l3 * PR * N1 + (long)first_cells * O * N1, src + l3 * N2 * N1,
+                         (uint32_t)((size_t)(RC - first_cells) * O * N1 * sizeof(T)), &full[slot]);
+        }
+    };
+    if (tid == 0)
+        for (int j = 0; j < NS && j < n3; ++j) issue(j);
+
+    // (k1,k2)-swept values of this thread's cell from a staged array with `rows` rows per x_3-node
+    auto k12_from = [&](const T *sl, long rows, T (&w)[O][O][O]) {
+#pragma unroll
+        for (int l3 = 0; l3 < O; ++l3) {
+            T tk[2][O][O];
+#pragma unroll
+            for (int e2 = 0; e2 < 2; ++e2)
+#pragma unroll
+                for (int l2 = 0; l2 < O; ++l2) {
+                    T r0[O], r1[O];
+                    load_cell<T, O>(sl + l3 * rows * N1 + off[e2][0] + l2 * N1, r0);
+                    load_cell<T, O>(sl + l3 * rows * N1 + off[e2][1] + l2 * N1, r1);
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) tk[e2][l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+                }
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a0[O], a1[O];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) { a0[l] = tk[0][l][j1]; a1[l] = tk[1][l][j1]; }
+                    w[l3][j2][j1] = chain<T, O>(A2, B2, j2, a0, a1);
+                }
+        }
+    };
+    auto a_half = [&](const T (&w)[O][O][O], T (&acc)[O][O][O]) {
+#pragma unroll
+        for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a = mul_t<T>(A3[j3 * O], w[0][j2][j1]);
+#pragma unroll
+                    for (int l = 1; l < O; ++l) a = fma_t<T>(A3[j3 * O + l], w[l][j2][j1], a);
+                    acc[j3][j2][j1] = a;
+                }
+    };
+    // B-half of the k3 rule; the O^3 results go to dst as O^2 rows of O values (row pitch N1, x_3-node pitch p3)
+    auto b_half_put = [&](const T (&acc)[O][O][O], const T (&w)[O][O][O], T *dst, long p3) {
+#pragma unroll
+        for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2) {
+                T res[O];
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a = acc[j3][j2][j1];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) a = fma_t<T>(B3[j3 * O + l], w[l][j2][j1], a);
+                    res[j1] = a;
+                }
+                T *p = dst + (long)j3 * p3 + (long)j2 * N1;
+                if constexpr (O % 2 == 0) {
+                    using V2 = Vec<T, 2>;
+#pragma unroll
+                    for (int j1 = 0; j1 < O; j1 += 2) {
+                        V2 vv; vv.v[0] = res[j1]; vv.v[1] = res[j1 + 1];
+                        *reinterpret_cast<V2 *>(p + j1) = vv;
+                    }
+                } else {
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) p[j1] = res[j1];
+                }
+            }
+    };
+    auto park_put = [&](int which, const T (&w)[O][O][O]) {
+#pragma unroll
+        for (int a = 0; a < O; ++a)
+#pragma unroll
+            for (int b = 0; b < O; ++b)
+#pragma unroll
+                for (int d = 0; d < O; ++d) park[((which * O3) + (a * O + b) * O + d) * nthr + tid] = w[a][b][d];
+    };
+    auto park_get = [&](int which, T (&w)[O][O][O]) {
+#pragma unroll
+        for (int a = 0; a < O; ++a)
+#pragma unroll
+            for (int b = 0; b < O; ++b)
+#pragma unroll
+                for (int d = 0; d < O; ++d) w[a][b][d] = park[((which * O3) + (a * O + b) * O + d) * nthr + tid];
+    };
+    const long own_t = (long)t2c * O * N1 + (long)c1 * O;                    // this thread's cell in a T buffer
+    const long own_g = (long)(c2_0 + (act2 ? t2 : 0)) * O * N1 + (long)c1 * O;   // ... in a global slab
+    auto tb = [&](int i) -> T * { return tbuf0 + (size_t)(i & 1) * (tb_stride / sizeof(T)); };
+
+    T acc1[O][O][O], acc2[O][O][O];
+    auto out_cell = [&](int i) {                             // output x_3-cell closed when first-application cell i arrives
+        int cell = i - 1 - (APPS == 2 ? m3 : 0);
+        if (cell < 0) cell += n3;
+        return cell;
+    };
+    auto second = [&](int i) {                               // APPS == 2: second application on the first one's cell i
+        mbar_wait(&tbar[i & 1], (uint32_t)((i >> 1) & 1));
+        if (!act2) return;
+        T b[O][O][O];
+        k12_from(tb(i), TR, b);
+        if (i == 0) park_put(1, b);
+        else b_half_put(acc2, b, out + base + (long)out_cell(i) * slab + own_g, N2 * N1);
+        a_half(b, acc2);
+    };
+
+    for (int j = 0; j < n3; ++j) {
+        const int slot = j % NS;
+        mbar_wait(&full[slot], (uint32_t)((j / NS) & 1));
+        T w[O][O][O];
+        if (act1) k12_from(reinterpret_cast<const T *>(smem_raw + slot * slot_stride), PR, w);
+        __syncthreads();                                     // slab consumed; everybody is through iteration j - 1
+        if (tid == 0 && j + NS < n3) issue(j + NS);
+        if (j == 0) {
+            if (act1) { park_put(0, w); a_half(w, acc1); }
+        } else if constexpr (APPS == 1) {
+            if (act1) {
+                b_half_put(acc1, w, out + base + (long)(j - 1) * slab + own_g, N2 * N1);
+                a_half(w, acc1);
+            }
+        } else {
+            if (act1) {
+                b_half_put(acc1, w, tb(j - 1) + own_t, TR * N1);   // first application, cell j - 1
+                a_half(w, acc1);
+            }
+            mbar_arrive(&tbar[(j - 1) & 1]);
+            if (j >= 2) second(j - 2);
+        }
+    }
+    if constexpr (APPS == 1) {
+        if (act1) {
+            T wf[O][O][O];
+            park_get(0, wf);
+            b_half_put(acc1, wf, out + base + (long)(n3 - 1) * slab + own_g, N2 * N1);   // closes the periodic line
+        }
+    } else {
+        __syncthreads();
+        if (act1) {
+            T wf[O][O][O];
+            park_get(0, wf);
+            b_half_put(acc1, wf, tb(n3 - 1) + own_t, TR * N1);   // first application closes its line
+        }
+        mbar_arrive(&tbar[(n3 - 1) & 1]);
+        second(n3 - 2);
+        second(n3 - 1);
+        if (act2) {
+            T bf[O][O][O];
+            park_get(1, bf);
+            b_half_put(acc2, bf, out + base + (long)out_cell(n3) * slab + own_g, N2 * N1);
+        }
+    }
 }
 
 }  // namespace sldg

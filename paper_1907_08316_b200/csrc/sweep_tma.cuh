@@ -106,7 +106,9 @@ __device__ __forceinline__ void load_cell(const T *p, T (&u)[O]) {
 // JH = outputs per thread: JH == O is one thread per cell; at O >= 5 a cell's O outputs are split over
 // ceil(O / JH) threads, each holding only its JH rows of A and B (thread-per-cell needs 2 O^2 coefficient
 // registers: > 200 registers and 3.7 TB/s at O = 6; thread-per-node re-reads the 2 O inputs O times: 3.4 TB/s).
-template <typename T, int O, int JH = O>
+// TWICE: the sweep applied twice in shared memory before the copy out (x(tau) x(tau) of two consecutive Strang
+// steps, bit-identical to two launches; see sweep_xpair_plane2_kernel).
+template <typename T, int O, int JH = O, bool TWICE = false>
 __global__ void __launch_bounds__(256)
 sweep_x1_bulk_kernel(const T *__restrict__ in, T *__restrict__ out, int n, long lines_per_group, int R,
                      int chunks_per_group, const int *__restrict__ mtab, const T *__restrict__ ab,
@@ -149,31 +151,38 @@ sweep_x1_bulk_kernel(const T *__restrict__ in, T *__restrict__ out, int n, long 
 #pragma unroll
         for (int e = 0; e < O * O; ++e) { A[e] = s_ab[e]; B[e] = s_ab[O * O + e]; }
         mbar_wait(&bar, 0);
-        for (int c = threadIdx.x; c < ncell; c += blockDim.x) {
-            const int line = c / n;
-            const int i = c - line * n;
-            int is = i + m;
-            if (is >= n) is -= n;
-            int is1 = is + 1;
-            if (is1 == n) is1 = 0;
-            T u0[O], u1[O];
-            load_cell<T, O>(s_in + (size_t)(line * n + is) * O, u0);
-            load_cell<T, O>(s_in + (size_t)(line * n + is1) * O, u1);
-            T r[O];
+        auto apply = [&](const T *src, T *dst) {
+            for (int c = threadIdx.x; c < ncell; c += blockDim.x) {
+                const int line = c / n;
+                const int i = c - line * n;
+                int is = i + m;
+                if (is >= n) is -= n;
+                int is1 = is + 1;
+                if (is1 == n) is1 = 0;
+                T u0[O], u1[O];
+                load_cell<T, O>(src + (size_t)(line * n + is) * O, u0);
+                load_cell<T, O>(src + (size_t)(line * n + is1) * O, u1);
+                T r[O];
 #pragma unroll
-            for (int j = 0; j < O; ++j) r[j] = chain<T, O>(A, B, j, u0, u1);
-            T *po = s_out + (size_t)c * O;
-            if constexpr (O % 2 == 0) {
-                using V2 = Vec<T, 2>;
+                for (int j = 0; j < O; ++j) r[j] = chain<T, O>(A, B, j, u0, u1);
+                T *po = dst + (size_t)c * O;
+                if constexpr (O % 2 == 0) {
+                    using V2 = Vec<T, 2>;
 #pragma unroll
-                for (int j = 0; j < O; j += 2) {
-                    V2 t; t.v[0] = r[j]; t.v[1] = r[j + 1];
-                    *reinterpret_cast<V2 *>(po + j) = t;
+                    for (int j = 0; j < O; j += 2) {
+                        V2 t; t.v[0] = r[j]; t.v[1] = r[j + 1];
+                        *reinterpret_cast<V2 *>(po + j) = t;
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < O; ++j) po[j] = r[j];
                 }
-            } else {
-#pragma unroll
-                for (int j = 0; j < O; ++j) po[j] = r[j];
             }
+        };
+        apply(s_in, s_out);
+        if constexpr (TWICE) {
+            __syncthreads();
+            apply(s_out, s_in);
         }
     } else {
         // work item = (cell, part): part p computes the outputs j = p*JH .. min(O, (p+1)*JH) - 1
@@ -188,39 +197,47 @@ sweep_x1_bulk_kernel(const T *__restrict__ in, T *__restrict__ out, int n, long 
             for (int l = 0; l < O; ++l) { Ar[jj][l] = s_ab[j * O + l]; Br[jj][l] = s_ab[O * O + j * O + l]; }
         }
         mbar_wait(&bar, 0);
-        for (int c = threadIdx.x / NP; c < ncell; c += blockDim.x / NP) {
-            const int line = c / n;
-            const int i = c - line * n;
-            int is = i + m;
-            if (is >= n) is -= n;
-            int is1 = is + 1;
-            if (is1 == n) is1 = 0;
-            T u0[O], u1[O];
-            load_cell<T, O>(s_in + (size_t)(line * n + is) * O, u0);
-            load_cell<T, O>(s_in + (size_t)(line * n + is1) * O, u1);
-            T *po = s_out + (size_t)c * O + jb;
+        auto apply = [&](const T *src, T *dst) {
+            for (int c = threadIdx.x / NP; c < ncell; c += blockDim.x / NP) {
+                const int line = c / n;
+                const int i = c - line * n;
+                int is = i + m;
+                if (is >= n) is -= n;
+                int is1 = is + 1;
+                if (is1 == n) is1 = 0;
+                T u0[O], u1[O];
+                load_cell<T, O>(src + (size_t)(line * n + is) * O, u0);
+                load_cell<T, O>(src + (size_t)(line * n + is1) * O, u1);
+                T *po = dst + (size_t)c * O + jb;
 #pragma unroll
-            for (int jj = 0; jj < JH; ++jj) {
-                T acc = mul_t<T>(Ar[jj][0], u0[0]);           // the O7 chain of output jb + jj
+                for (int jj = 0; jj < JH; ++jj) {
+                    T acc = mul_t<T>(Ar[jj][0], u0[0]);       // the O7 chain of output jb + jj
 #pragma unroll
-                for (int l = 1; l < O; ++l) acc = fma_t<T>(Ar[jj][l], u0[l], acc);
+                    for (int l = 1; l < O; ++l) acc = fma_t<T>(Ar[jj][l], u0[l], acc);
 #pragma unroll
-                for (int l = 0; l < O; ++l) acc = fma_t<T>(Br[jj][l], u1[l], acc);
-                if (jb + jj < O) po[jj] = acc;
+                    for (int l = 0; l < O; ++l) acc = fma_t<T>(Br[jj][l], u1[l], acc);
+                    if (jb + jj < O) po[jj] = acc;
+                }
             }
+        };
+        apply(s_in, s_out);
+        if constexpr (TWICE) {
+            __syncthreads();
+            apply(s_out, s_in);
         }
     }
+    const T *s_res = TWICE ? s_in : s_out;                   // where the result sits
     fence_proxy_async();
     __syncthreads();
     if (contiguous) {
         if (threadIdx.x == 0) {
-            bulk_s2g(out + base, s_out, bytes);
+            bulk_s2g(out + base, s_res, bytes);
             bulk_commit();
             bulk_wait_read0();
         }
     } else {
         for (int r = threadIdx.x; r < nl; r += blockDim.x) {
-            bulk_s2g(out + base + r * line_stride, s_out + (size_t)r * n * O, line_bytes);
+            bulk_s2g(out + base + r * line_stride, s_res + (size_t)r * n * O, line_bytes);
             bulk_commit();
             bulk_wait_read0();
         }

@@ -18,7 +18,7 @@ EXPORTS = [
     "sldg_create", "sldg_destroy", "sldg_last_error", "sldg_num_dofs", "sldg_num_x",
     "sldg_node_coords", "sldg_set_initial", "sldg_get_f", "sldg_current", "sldg_fill_uniform",
     "sldg_translate", "sldg_translate_dev", "sldg_advect", "sldg_advect_pair", "sldg_translate_pair_dev", "sldg_advect_triple", "sldg_translate_triple_dev", "sldg_compute_rho", "sldg_poisson_E",
-    "sldg_set_E", "sldg_advect_x_rho", "sldg_step", "sldg_diagnostics", "sldg_moments", "sldg_invariants", "sldg_launch_count",
+    "sldg_set_E", "sldg_advect_x_rho", "sldg_advect_x_twice", "sldg_step", "sldg_step_n", "sldg_diagnostics", "sldg_moments", "sldg_invariants", "sldg_launch_count",
 ]
 
 
@@ -55,6 +55,8 @@ def _load():
     lib.sldg_set_E.argtypes = [vp, vp, C.c_int]
     lib.sldg_step.argtypes = [vp, C.c_double]
     lib.sldg_advect_x_rho.argtypes = [vp, C.c_double, vp]
+    lib.sldg_advect_x_twice.argtypes = [vp, C.c_double]
+    lib.sldg_step_n.argtypes = [vp, C.c_double, C.c_int]
     lib.sldg_diagnostics.argtypes = [vp, dp, dp, dp]
     lib.sldg_moments.argtypes = [vp, dp, dp]
     lib.sldg_invariants.argtypes = [vp, dp, dp, dp, dp, dp]
@@ -227,6 +229,13 @@ class Sldg:
         rho = self.torch.empty(self.X, dtype=self.torch.float64, device=self.device)
         self._chk(_lib.sldg_advect_x_rho(self.h, float(tau), rho.data_ptr()), "advect_x_rho")
         return rho
+
+    def advect_x_twice(self, tau):
+        self._chk(_lib.sldg_advect_x_twice(self.h, float(tau)), "advect_x_twice")
+
+    def step_n(self, dt, nsteps):
+        """nsteps Strang steps with the x half-steps of consecutive steps merged into one pass."""
+        self._chk(_lib.sldg_step_n(self.h, float(dt), int(nsteps)), "step_n")
 
     def step(self, dt):
         self._chk(_lib.sldg_step(self.h, float(dt)), "step")

@@ -250,6 +250,97 @@ def test_advect_x_rho_is_the_sweeps_plus_rho(oracle, monkeypatch, shape, cells_e
     a.close(); b.close()
 
 
+def _x_group(s, dx, o, tau):
+    if dx == 3 and o <= 2:
+        s.advect_triple(0, 1, 2, tau)
+    elif dx >= 2 and o <= 4:
+        s.advect_pair(0, 1, tau)
+        for d in range(2, dx):
+            s.advect(d, tau)
+    else:
+        for d in range(dx):
+            s.advect(d, tau)
+
+
+_X2_SHAPES = [(1, 1, (16, 12), 3), (1, 1, (9, 7), 6), (1, 3, (8, 5, 4, 3), 4), (2, 2, (16, 16, 6, 5), 2),
+              (2, 2, (12, 9, 5, 4), 3), (2, 2, (8, 7, 4, 3), 4), (2, 2, (8, 3, 4, 3), 1),
+              (3, 3, (6, 5, 7, 3, 4, 3), 2), (3, 3, (4, 4, 11, 3, 3, 2), 1),
+              (2, 3, (8, 8, 3, 4, 3), 2), (3, 3, (4, 4, 4, 3, 3, 3), 3),
+              (3, 3, (6, 6, 5, 3, 4, 3), 2), (3, 3, (5, 8, 4, 3, 3, 3), 2)]
+# SLDG_XTRIPLE_PARTS (whole-plane / part-plane x-triple kernels) only concerns d_x = 3
+_X2_CASES = [(sh, "") for sh in _X2_SHAPES] + [(sh, p) for sh in _X2_SHAPES if sh[0] == 3 for p in ("1", "2")]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape,parts", _X2_CASES)
+def test_advect_x_twice_is_bitwise_the_group_twice(monkeypatch, shape, parts, dtype):
+    """x(tau) x(tau) in one pass (sldg_advect_x_twice: the merged half-steps of sldg_step_n) against the x-group
+    issued twice through the public calls, bit for bit; covers the one-pass kernels (bulk x_1, plane pair,
+    plane triple) and the shapes that fall back to two passes."""
+    dx, dv, cells, o = shape
+    if parts:
+        monkeypatch.setenv("SLDG_XTRIPLE_PARTS", parts)
+    lo = (0.0,) * dx + (-4.0, -3.0, -5.0)[:dv]
+    hi = tuple(2 * np.pi * (1 + 0.5 * a) for a in range(dx)) + (4.5, 3.5, 4.0)[:dv]
+    cfg = W.Config("x2", dx, dv, cells, o, lo, hi)
+    rng = np.random.default_rng(33)
+    f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
+    tau = 0.61
+    a = make_solver(cfg, dtype)
+    a.set_initial(f0)
+    l0 = a.launch_count()
+    a.advect_x_twice(tau)
+    la = a.launch_count() - l0
+    fa = a.get_f()
+    b = make_solver(cfg, dtype)
+    b.set_initial(f0)
+    l0 = b.launch_count()
+    _x_group(b, dx, o, tau)
+    _x_group(b, dx, o, tau)
+    lb = b.launch_count() - l0
+    fb = b.get_f()
+    a.close(); b.close()
+    assert np.array_equal(fa, fb)
+    assert la <= lb
+    if shape in ((1, 1, (16, 12), 3), (2, 2, (16, 16, 6, 5), 2), (3, 3, (6, 5, 7, 3, 4, 3), 2)):
+        assert la < lb                                  # these take the one-pass kernels
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(1, 1, (16, 12), 3), (2, 2, (12, 8, 6, 5), 2), (2, 2, (10, 6, 5, 4), 3),
+                                   (3, 3, (5, 4, 6, 3, 4, 3), 2), (1, 3, (8, 5, 4, 3), 4), (2, 3, (6, 6, 3, 4, 3), 4)])
+def test_step_n_is_n_steps(oracle, monkeypatch, shape, dtype):
+    """sldg_step_n (x half-steps of consecutive steps merged) against n calls of sldg_step: bit for bit when rho
+    is its own pass in both (SLDG_NO_FUSE_RHO=1), at rounding level with the default fused rho; and against the
+    oracle's n steps within the north-star tolerance."""
+    dx, dv, cells, o = shape
+    monkeypatch.setenv("SLDG_NO_GRAPH", "1")          # small test shapes would otherwise replay the one-step graph
+    cfg = W.Config("sn", dx, dv, cells, o, (0.0,) * dx + (-6.0,) * dv, (4 * np.pi,) * dx + (6.0,) * dv, dt=0.1,
+                   kind="landau", eps=0.05, k=0.5)
+    g = _grid(oracle, cfg)
+    f0 = W.initial_state(cfg, [g.coords(d) for d in range(dx + dv)], NPDT[dtype])
+    n = 4
+    outs = {}
+    for norho in ("1", "0"):
+        monkeypatch.setenv("SLDG_NO_FUSE_RHO", norho)
+        a = make_solver(cfg, dtype); a.set_initial(f0)
+        l0 = a.launch_count(); a.step_n(cfg.dt, n); la = a.launch_count() - l0
+        b = make_solver(cfg, dtype); b.set_initial(f0)
+        l0 = b.launch_count()
+        for _ in range(n):
+            b.step(cfg.dt)
+        lb = b.launch_count() - l0
+        outs[norho] = (a.get_f(), b.get_f(), la, lb)
+        a.close(); b.close()
+    assert np.array_equal(outs["1"][0], outs["1"][1])
+    assert outs["1"][2] <= outs["1"][3]
+    assert rel_err(outs["0"][0], outs["0"][1]) <= (1e-13 if dtype == "f64" else 1e-5)
+    ref = f0.copy()
+    for _ in range(n):
+        g.step(ref, cfg.dt)
+    assert rel_err(outs["0"][0], ref) <= TOL[dtype]
+
+
 def test_config1_momentum_and_total_energy_on_the_gpu(oracle):
     cfg = W.CONFIG1
     s = make_solver(cfg, "f64")
