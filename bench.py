@@ -28,10 +28,10 @@ sys.path.insert(0, ROOT)
 from paper_1907_08316_b200 import workloads as W  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the sweep kernel of each direction, from one
-# ncu capture of this very command at full size (profiles/traffic_fullsize_r1c.md); None where not captured.
+# ncu capture of this very command at full size (profiles/traffic_launches_r2.md); None where not captured.
 TRAFFIC_BYTES = {
-    ("config4-sweep-2+2", "f64"): {0: 43.489e9 + 43.437e9, 1: 43.830e9 + 43.439e9,
-                                   2: 43.703e9 + 43.428e9, 3: 43.698e9 + 43.428e9},
+    ("config4-sweep-2+2", "f64"): {0: 43.497e9 + 43.436e9, 1: 43.829e9 + 43.445e9,
+                                   2: 43.520e9 + 43.432e9, 3: 43.520e9 + 43.433e9},
 }
 
 METRIC = "achieved_hbm_gbs_per_translation_sweep"
@@ -323,6 +323,14 @@ def strang_step_table(torch, Sldg, cfg, dtype, steps):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
     launches_per_step = (s.launch_count() - l0) / steps
+    # the same steps with the x half-steps of consecutive steps merged into one pass (sldg_step_n; same f)
+    e2 = torch.cuda.Event(enable_timing=True); e3 = torch.cuda.Event(enable_timing=True)
+    s.step_n(cfg.dt, 2)
+    e2.record()
+    s.step_n(cfg.dt, steps)
+    e3.record()
+    torch.cuda.synchronize()
+    ms_merged = e2.elapsed_time(e3) / steps
     # the paper's own loop writes the invariants once per step: one more read of f (sldg_invariants)
     t0 = time.perf_counter()
     for _ in range(steps):
@@ -333,7 +341,9 @@ def strang_step_table(torch, Sldg, cfg, dtype, steps):
     es = 8 if dtype == "f64" else 4
     passes = 2 * (3 * cfg.dx) + 1
     mass, l2, ee = s.diagnostics()
-    out = {"ms_per_step": ms, "ms_per_step_with_invariants_every_step": ms_inv, "passes_paper_accounting": passes,
+    out = {"ms_per_step": ms, "ms_per_step_merged_half_steps": ms_merged,
+           "gbs_paper_eq1_style_merged": passes * cfg.ndof * es / ms_merged / 1e6,
+           "ms_per_step_with_invariants_every_step": ms_inv, "passes_paper_accounting": passes,
            "gbs_paper_eq1_style_with_invariants": (passes + 1) * cfg.ndof * es / ms_inv / 1e6,
            "gbs_paper_eq1_style": passes * cfg.ndof * es / ms / 1e6,
            "dof_updates_per_s": 3 * cfg.dx * cfg.ndof / ms * 1e3,
@@ -438,7 +448,7 @@ def run_ours(args):
     roofline = {"bound": "hbm", "achieved": sweep_bytes / dim_avg[dom] / 1e6, "peak": peak, "unit": "GB/s",
                 "frac": sweep_bytes / dim_avg[dom] / 1e6 / peak,
                 "traffic": TRAFFIC_BYTES.get((cfg.name, dtype), {}).get(dom),
-                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/traffic_fullsize_r1c.md",
+                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/traffic_launches_r2.md",
                 "kernel": "translation sweep along dim %d (slowest direction)" % dom,
                 "algorithmic_bytes_per_launch": sweep_bytes, "peak_source": peak_src,
                 "per_direction_gbs": {"dim%d" % d: sweep_bytes / t / 1e6 for d, t in dim_avg.items()},

@@ -638,7 +638,7 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
             if (ts.valid) {
                 const CUtensorMap &tmap = ts.map;
                 CUDA_TRY(c, ensure_smem(c, sweep_tile_tma_kernel<T, O>, smem));
-                int nseg = 128 / W;
+                int nseg = 128 / W;                       // (256 / 512 threads per tile measured: 1-2 % / 15 % slower)
                 int cps = (int)cdiv(n, nseg);
                 long tpo = cdiv(inner, W);
                 sweep_tile_tma_kernel<T, O><<<(unsigned)(tpo * outer), 128, smem, c->stream>>>(
@@ -1035,7 +1035,15 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
         case 6: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 4, 2, 1, true>, 32, 4, 2); break;
         case 7: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 2, 2, false, false>, 32, 2, 2); break;
         case 8: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 1, 2, 4, false>, 32, 1, 2); break;
-        default: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 2, 2, false>, 32, 2, 2); break;   // two resident blocks of 4 x 2 cells: 14.8 -> 13.9 ms at config 5
+        case 9: rc = launch(sweep_vtriple_tile_kernel<T, O, 64, 2, 2, 1, false>, 64, 2, 2); break;
+        case 10: rc = launch(sweep_vtriple_tile_kernel<T, O, 64, 1, 2, 2, false>, 64, 1, 2); break;
+        case 11: rc = launch(sweep_vtriple_tile_kernel<T, O, 64, 1, 3, 2, false>, 64, 1, 3); break;
+        default:
+            // fp32: 64 columns keep the rows at 256 bytes (9.3 -> 8.5 ms at config 5); fp64: two resident blocks of
+            // 4 x 2 cells (14.8 -> 13.9 ms)
+            if (sizeof(T) == 4) rc = launch(sweep_vtriple_tile_kernel<T, O, 64, 1, 2, 2, false>, 64, 1, 2);
+            if (rc) rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 2, 2, false>, 32, 2, 2);
+            break;
         }
         if (rc == 0) {
             LAUNCH_CHECK(c);

@@ -3,11 +3,12 @@ buckets of the paper's Fig. 5 ("advection x", "compute r
 "advection v").
 
     python -m paper_1907_08316_b200.examples.strang_steps --config config5 [--steps 5] [--warmup 2]
-           [--dtype f64] [--order O] [--cells n1,n2,..] [--buckets] [--diagnostics]
+           [--dtype f64] [--order O] [--cells n1,n2,..] [--buckets] [--diagnostics] [--merged]
 
 --config: config1 | config2 | config3 | config5 | mixed13 | mixed23 | twostream (the paper's eq. (2) run).
 --buckets issues the same sequence as sldg_step through the public calls (advect pair/triple, compute_rho,
 poisson_E) with CUDA events between the categories; without it the step is one sldg_step call.
+--merged runs the steps as ONE sldg_step_n call (the x half-steps of consecutive steps in one pass).
 --diagnostics adds sldg_diagnostics + sldg_moments after every step (the paper writes its invariants
 every step), i.e. the "14 passes" accounting of its eq. (1).
 Prints one JSON line.  Every step runs in the CUDA library; torch only builds the initial state.
@@ -52,7 +53,7 @@ def advect_group(s, base, cnt, tau):
         s.advect(base, tau)
 
 
-def run(cfg, dtype="f64", steps=5, warmup=2, buckets=False, diagnostics=False):
+def run(cfg, dtype="f64", steps=5, warmup=2, buckets=False, diagnostics=False, merged=False):
     import torch
     s = Sldg.from_config(cfg, dtype=dtype)
     device_initial_state(torch, s, cfg)
@@ -83,8 +84,11 @@ def run(cfg, dtype="f64", steps=5, warmup=2, buckets=False, diagnostics=False):
     l0 = s.launch_count()
     e0.record()
     last = None
-    for _ in range(steps):
-        last = one(ev)
+    if merged and not buckets and not diagnostics:
+        s.step_n(cfg.dt, steps)
+    else:
+        for _ in range(steps):
+            last = one(ev)
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
@@ -97,7 +101,7 @@ def run(cfg, dtype="f64", steps=5, warmup=2, buckets=False, diagnostics=False):
     passes = 2 * (2 * cfg.dx + cfg.dx) + 1 + (1 if diagnostics else 0)   # paper eq. (1) accounting
     mass, l2, ee = s.diagnostics()
     out = {"config": cfg.name, "cells": list(cfg.cells), "order": cfg.order, "dtype": dtype, "ndof": cfg.ndof,
-           "steps": steps, "ms_per_step": ms, "passes_paper_accounting": passes,
+           "steps": steps, "merged_half_steps": bool(merged), "ms_per_step": ms, "passes_paper_accounting": passes,
            "gbs_paper_eq1_style": passes * cfg.ndof * es / ms / 1e6,
            "launches_per_step": (s.launch_count() - l0) / steps,
            "mass": mass, "l2": l2, "electric_energy": ee}
@@ -119,10 +123,11 @@ def main():
     ap.add_argument("--cells", default=None, help="comma-separated cell counts (default: the config's)")
     ap.add_argument("--buckets", action="store_true")
     ap.add_argument("--diagnostics", action="store_true")
+    ap.add_argument("--merged", action="store_true")
     a = ap.parse_args()
     cells = tuple(int(c) for c in a.cells.split(",")) if a.cells else None
     cfg = make_config(a.config, cells, a.order)
-    print(json.dumps(run(cfg, a.dtype, a.steps, a.warmup, a.buckets, a.diagnostics)))
+    print(json.dumps(run(cfg, a.dtype, a.steps, a.warmup, a.buckets, a.diagnostics, a.merged)))
 
 
 if __name__ == "__main__":

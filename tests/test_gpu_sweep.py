@@ -402,19 +402,28 @@ def test_tile_staged_v_pair(oracle, o, dtype, kind, monkeypatch):
         sig[1][cfg.X - 7] = -1.7
     a = make_solver(cfg, dtype)
     a.set_initial(f0)
-    a.translate_pair(2, torch.from_numpy(sig[0]).cuda(), 3, torch.from_numpy(sig[1]).cuda())
-    fused = a.get_f()
-    a.close()
     b = make_solver(cfg, dtype)
     b.set_initial(f0)
-    b.translate(2, sig[0])
-    b.translate(3, sig[1])
-    seq = b.get_f()
-    b.close()
-    assert np.array_equal(fused, seq)
     ref = f0.copy()
-    oracle.translate(ref, cfg.N, cfg.order, 2, sig[0], [0, 1])
-    oracle.translate(ref, cfg.N, cfg.order, 3, sig[1], [0, 1])
+    if kind == "some-large":
+        # the raw call would route shifts of a cell or more to single sweeps (sldg.h); the physics call does not
+        # check, so it reaches the kernel's per-block fallback: sigma = -E dt / h_v with dt = 1
+        g = oracle.Grid(cfg.dx, cfg.dv, cfg.cells, cfg.order, cfg.lo, cfg.hi)
+        E = np.stack([-sig[a_] * (cfg.hi[2 + a_] - cfg.lo[2 + a_]) / cfg.cells[2 + a_] for a_ in range(2)])
+        a.set_E(E); b.set_E(E)
+        a.advect_pair(2, 3, 1.0)
+        b.advect(2, 1.0); b.advect(3, 1.0)
+        g.advect(ref, 2, 1.0, E); g.advect(ref, 3, 1.0, E)
+    else:
+        a.translate_pair(2, torch.from_numpy(sig[0]).cuda(), 3, torch.from_numpy(sig[1]).cuda())
+        b.translate(2, sig[0])
+        b.translate(3, sig[1])
+        oracle.translate(ref, cfg.N, cfg.order, 2, sig[0], [0, 1])
+        oracle.translate(ref, cfg.N, cfg.order, 3, sig[1], [0, 1])
+    fused = a.get_f()
+    seq = b.get_f()
+    a.close(); b.close()
+    assert np.array_equal(fused, seq)
     assert rel_err(fused, ref) <= TOL[dtype]
 
 
@@ -439,18 +448,26 @@ def test_tile_staged_v_triple(oracle, o, dtype, kind):
             sig[2][cfg.X - 7] = -1.7
     a = make_solver(cfg, dtype)
     a.set_initial(f0)
-    a.translate_triple(3, torch.from_numpy(sig[0]).cuda(), 4, torch.from_numpy(sig[1]).cuda(),
-                       5, torch.from_numpy(sig[2]).cuda())
-    fused = a.get_f()
-    a.close()
     b = make_solver(cfg, dtype)
     b.set_initial(f0)
-    for k, s_ in zip((3, 4, 5), sig):
-        b.translate(k, s_)
-    seq = b.get_f()
-    b.close()
-    assert np.array_equal(fused, seq)
     ref = f0.copy()
-    for k, s_ in zip((3, 4, 5), sig):
-        oracle.translate(ref, cfg.N, cfg.order, k, s_, [0, 1, 2])
+    if kind == "some-large":
+        # physics call (no routing of wide shifts): reaches the kernel's per-block fallback
+        g = oracle.Grid(cfg.dx, cfg.dv, cfg.cells, cfg.order, cfg.lo, cfg.hi)
+        E = np.stack([-sig[a_] * (cfg.hi[3 + a_] - cfg.lo[3 + a_]) / cfg.cells[3 + a_] for a_ in range(3)])
+        a.set_E(E); b.set_E(E)
+        a.advect_triple(3, 4, 5, 1.0)
+        for k in (3, 4, 5):
+            b.advect(k, 1.0)
+            g.advect(ref, k, 1.0, E)
+    else:
+        a.translate_triple(3, torch.from_numpy(sig[0]).cuda(), 4, torch.from_numpy(sig[1]).cuda(),
+                           5, torch.from_numpy(sig[2]).cuda())
+        for k, s_ in zip((3, 4, 5), sig):
+            b.translate(k, s_)
+            oracle.translate(ref, cfg.N, cfg.order, k, s_, [0, 1, 2])
+    fused = a.get_f()
+    seq = b.get_f()
+    a.close(); b.close()
+    assert np.array_equal(fused, seq)
     assert rel_err(fused, ref) <= TOL[dtype]
