@@ -938,7 +938,7 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
                 //  of cells redundantly: 22.9 ms against 21.1 ms for the whole plane, so twice stays on whole planes
                 //  unless SLDG_XTRIPLE_PARTS asks otherwise)
                 const int nb2 = c->tune.xt_parts ? c->tune.xt_parts : (c->twice_req ? 1 : 2);
-                const int apps = c->twice_req ? 2 : 1;
+                const int apps = (c->twice_req && n3 >= 2) ? 2 : 1;
                 if (nb2 >= 2 && n2 % nb2 == 0 && n2 / nb2 >= 2) {
                     const int c2b = n2 / nb2;
                     const long thr = (long)(c2b + apps - 1) * n1;
@@ -983,7 +983,7 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
             int block = (int)(cdiv((long)tpr * n2, 32) * 32);
             // twice: ring + the first application's cell + the two parked first cells of the windows
             const size_t smem2 = 5 * slot + (size_t)2 * O * O * O * block * sizeof(T);   // 3-deep ring, 2 cells, parked
-            if (c->twice_req && smem2 <= 226 * 1024 &&
+            if (c->twice_req && n3 >= 2 && smem2 <= 226 * 1024 &&
                 ensure_smem(c, sweep_xtriple_plane2_kernel<T, O>, smem2) == cudaSuccess) {
                 sweep_xtriple_plane2_kernel<T, O><<<(unsigned)outer3, block, smem2, c->stream>>>(
                     in, out, n1, n2, n3, tpr, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1], (const T *)ab[1], cnt2,

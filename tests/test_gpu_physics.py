@@ -266,7 +266,8 @@ _X2_SHAPES = [(1, 1, (16, 12), 3), (1, 1, (9, 7), 6), (1, 3, (8, 5, 4, 3), 4), (
               (2, 2, (12, 9, 5, 4), 3), (2, 2, (8, 7, 4, 3), 4), (2, 2, (8, 3, 4, 3), 1),
               (3, 3, (6, 5, 7, 3, 4, 3), 2), (3, 3, (4, 4, 11, 3, 3, 2), 1),
               (2, 3, (8, 8, 3, 4, 3), 2), (3, 3, (4, 4, 4, 3, 3, 3), 3),
-              (3, 3, (6, 6, 5, 3, 4, 3), 2), (3, 3, (5, 8, 4, 3, 3, 3), 2)]
+              (3, 3, (6, 6, 5, 3, 4, 3), 2), (3, 3, (5, 8, 4, 3, 3, 3), 2),
+              (3, 3, (4, 4, 2, 3, 3, 3), 2), (3, 3, (4, 4, 1, 3, 3, 3), 2), (2, 2, (8, 3, 4, 3), 2), (1, 1, (1, 5), 2)]
 # SLDG_XTRIPLE_PARTS (whole-plane / part-plane x-triple kernels) only concerns d_x = 3
 _X2_CASES = [(sh, "") for sh in _X2_SHAPES] + [(sh, p) for sh in _X2_SHAPES if sh[0] == 3 for p in ("1", "2")]
 
