@@ -1026,18 +1026,12 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
         };
         int rc = 1;
         switch (c->tune.vt_variant) {
+        // kept for A/B runs (DESIGN.md section 5 lists what the others measured): 0 = round-1 geometry (one block of
+        // 4 x 4 cells), 1 = the same with per-warp slot release and a 3-deep ring, 2 = fp64 default, 10 = fp32 default
         case 0: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 4, 2, 1, false>, 32, 4, 2); break;
         case 1: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 4, 3, 1, true>, 32, 4, 3); break;
         case 2: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 2, 2, false>, 32, 2, 2); break;
-        case 3: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 3, 2, true>, 32, 2, 3); break;
-        case 4: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 4, 3, 2, false>, 16, 4, 3); break;
-        case 5: rc = launch(sweep_vtriple_tile_kernel<T, O, 16, 4, 4, 2, true>, 16, 4, 4); break;
-        case 6: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 4, 2, 1, true>, 32, 4, 2); break;
-        case 7: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 2, 2, false, false>, 32, 2, 2); break;
-        case 8: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 1, 2, 4, false>, 32, 1, 2); break;
-        case 9: rc = launch(sweep_vtriple_tile_kernel<T, O, 64, 2, 2, 1, false>, 64, 2, 2); break;
         case 10: rc = launch(sweep_vtriple_tile_kernel<T, O, 64, 1, 2, 2, false>, 64, 1, 2); break;
-        case 11: rc = launch(sweep_vtriple_tile_kernel<T, O, 64, 1, 3, 2, false>, 64, 1, 3); break;
         default:
             // fp32: 64 columns keep the rows at 256 bytes (9.3 -> 8.5 ms at config 5); fp64: two resident blocks of
             // 4 x 2 cells (14.8 -> 13.9 ms)
