@@ -52,6 +52,8 @@ struct sldg_ctx {
         bool tile_triple = true;       // SLDG_NO_TILE_TRIPLE=1 -> false
         int vt_variant = -1;           // SLDG_VTRIPLE_VARIANT: staged v-triple variant (-1 = default)
         int xt_parts = 0;              // SLDG_XTRIPLE_PARTS: x_2-ranges per velocity node in the x-triple (0 = default, 1 = whole plane)
+        bool xt_two = true;            // SLDG_XTRIPLE_ONE=1 -> false: one x_2-cell per thread in the part-plane x-triple
+        bool twice_triple = false;     // SLDG_TWICE_TRIPLE=1: sldg_step_n also merges the x half-steps in 3+3 D (slower, section 9)
         bool twice = true;             // SLDG_NO_TWICE=1 -> false: sldg_step_n never merges the x half-steps of two steps
         bool fuse_rho = true;          // SLDG_NO_FUSE_RHO=1 -> false: rho is a pass of its own after the x-group
         bool rho_triple = false;       // SLDG_RHO_TRIPLE=1: also fuse rho into the x-triple (3+3 D: measured break-even, off)
@@ -284,6 +286,8 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         c->tune.vt_variant = env_int("SLDG_VTRIPLE_VARIANT", -1, 0, 15);
         c->tune.fuse_rho = !env_flag("SLDG_NO_FUSE_RHO");
         c->tune.twice = !env_flag("SLDG_NO_TWICE");
+        c->tune.xt_two = !env_flag("SLDG_XTRIPLE_ONE");
+        c->tune.twice_triple = env_flag("SLDG_TWICE_TRIPLE");
         c->tune.xt_parts = env_int("SLDG_XTRIPLE_PARTS", 0, 1, 8);
         c->tune.rho_triple = env_flag("SLDG_RHO_TRIPLE");
         c->tune.rho_cells = env_int("SLDG_RHO_CELLS", 0, 1, 8);
@@ -934,9 +938,10 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
             4 * slot <= 200 * 1024 && (long)n1 * n2 <= 512 && outer3 < (1L << 31)) {
             // Part-plane blocks (nb2 ranges of x_2-cells per velocity node): two resident blocks whose phases overlap
             {
-                // (config 5: single application 12.2 -> 11.5 ms; applied twice the part kernel spills and computes a row
-                //  of cells redundantly: 22.9 ms against 21.1 ms for the whole plane, so twice stays on whole planes
-                //  unless SLDG_XTRIPLE_PARTS asks otherwise)
+                // (config 5: single application 12.2 -> 11.5 ms, and -> 9.9 ms with two x_2-cells per thread
+                //  (sweep_xtriple_part2_kernel); applied twice the part kernel spills and computes a row of cells
+                //  redundantly: 22.9 ms against 21.1 ms for the whole plane, so twice stays on whole planes unless
+                //  SLDG_XTRIPLE_PARTS asks otherwise -- and is off in 3+3 D, where two passes of 9.9 ms beat it)
                 const int nb2 = c->tune.xt_parts ? c->tune.xt_parts : (c->twice_req ? 1 : 2);
                 const int apps = (c->twice_req && n3 >= 2) ? 2 : 1;
                 if (nb2 >= 2 && n2 % nb2 == 0 && n2 / nb2 >= 2) {
@@ -955,6 +960,16 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
                             e = ensure_smem(c, kern, smem_p);
                             if (e == cudaSuccess)
                                 kern<<<(unsigned)(outer3 * nb2), blk, smem_p, c->stream>>>(
+                                    in, out, n1, n2, n3, c2b, nb2, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1],
+                                    (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+                        } else if (c2b % 2 == 0 && c->tune.xt_two) {
+                            // two x_2-cells per thread: half the threads, the shared source cell swept once
+                            auto kern = sweep_xtriple_part2_kernel<T, O>;
+                            const int blk2 = (int)(cdiv((long)(c2b / 2) * n1, 32) * 32);
+                            const size_t smem2c = 4 * slot_p + (size_t)2 * O * O * O * blk2 * sizeof(T);
+                            e = blk2 <= 128 ? ensure_smem(c, kern, smem2c) : cudaErrorInvalidValue;
+                            if (e == cudaSuccess)
+                                kern<<<(unsigned)(outer3 * nb2), blk2, smem2c, c->stream>>>(
                                     in, out, n1, n2, n3, c2b, nb2, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1],
                                     (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
                         } else {
@@ -1517,7 +1532,7 @@ int advect_group(sldg_ctx *c, int base, int cnt, double tau, bool with_rho = fal
     const bool whole = c->use_fuse && ((cnt == 3 && c->o <= 2) || (cnt == 2 && c->o <= 4));
     c->want_rho = with_rho && whole && c->tune.fuse_rho && base == 0;
     // twice: only a kernel that performs the WHOLE group may apply it twice in its pass (c->twice_done tells)
-    c->twice_req = twice && base == 0 && c->tune.twice && (whole || cnt == 1);
+    c->twice_req = twice && base == 0 && c->tune.twice && (whole || cnt == 1) && (cnt < 3 || c->tune.twice_triple);
     c->twice_done = false;
     struct Clear { sldg_ctx *c; ~Clear() { c->want_rho = false; c->twice_req = false; } } clear{c};
     if (c->use_fuse && cnt == 3 && c->o <= 2) return sldg_advect_triple(c, base, base + 1, base + 2, tau);

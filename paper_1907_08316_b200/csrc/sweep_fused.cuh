@@ -2035,3 +2035,194 @@ sweep_xtriple_part_kernel(const T *__restrict__ in, T *__restrict__ out, int n1,
 }
 
 }  // namespace sldg
+
+namespace sldg {
+
+// ------------------------------------------------------------------------------------------
+// sweep_xtriple_part_kernel<T, O, 1> with TWO adjacent x_2-cells per thread.  The k1-swept values of the x_2
+// source cell shared by the two output cells are computed once instead of twice: 12 instead of 16 shared-memory
+// loads and 28 instead of 32 FMA chains per output cell (the plane kernels are bound by exactly these two units,
+// and under the power cap every instruction saved is clock gained).  c2b must be even.  Same arithmetic per
+// value, bit-identical to the single sweeps.
+// ------------------------------------------------------------------------------------------
+template <typename T, int O>
+__global__ void __launch_bounds__(128, 3)
+sweep_xtriple_part2_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2, int n3, int c2b, int nb2,
+                           const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
+                           const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2,
+                           const int *__restrict__ mtab3, const T *__restrict__ ab3, long count3, long qdiv3, long qmod3) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    constexpr int NS = 4;
+    constexpr int O3 = O * O * O;
+    __shared__ __align__(8) uint64_t full[NS];
+    const long N1 = (long)n1 * O, N2 = (long)n2 * O;
+    const long slab = O * N2 * N1;                           // elements per x_3-cell of one node (global)
+    const int RC = c2b + 1;                                  // staged x_2-cells
+    const long PR = (long)RC * O;                            // staged rows per x_3-node
+    const long lslab = O * PR * N1;
+    const size_t slot_stride = ((size_t)lslab * sizeof(T) + 127) & ~(size_t)127;
+    T *park = reinterpret_cast<T *>(smem_raw + NS * slot_stride);   // [2][O3][blockDim]: the two windows' first cells
+    const long v = blockIdx.x / nb2;
+    const int c2_0 = (int)(blockIdx.x % nb2) * c2b;
+    const long base = v * (long)n3 * slab;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int c1 = tid % n1, tp = tid / n1;                  // tp: pair of x_2-cells 2 tp, 2 tp + 1 (local)
+    const bool active = 2 * tp < c2b;
+
+    const long q1 = (base / qdiv1) % qmod1, q2 = (base / qdiv2) % qmod2, q3 = (base / qdiv3) % qmod3;
+    T A1[O * O], B1[O * O], A2[O * O], B2[O * O], A3[O * O], B3[O * O];
+#pragma unroll
+    for (int e = 0; e < O * O; ++e) {
+        A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1];
+        A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
+        A3[e] = ab3[(long)e * count3 + q3]; B3[e] = ab3[(long)(O * O + e) * count3 + q3];
+    }
+    const int m1 = mtab1[q1], m2 = mtab2[q2], m3 = mtab3[q3];
+    int sa1 = c1 + m1; if (sa1 >= n1) sa1 -= n1;
+    int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
+    const int t2 = active ? 2 * tp : 0;
+    const int offa = (int)(t2 * O * N1 + sa1 * O), offb = (int)(t2 * O * N1 + sb1 * O);   // first of the 3 source cells
+    int rs = (c2_0 + m2) % n2;                               // first staged x_2-cell (global index)
+    const int first_cells = (rs + RC <= n2) ? RC : n2 - rs;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+    }
+    __syncthreads();
+    auto issue = [&](int j) {                                // slab j <-> source x_3-cell (m3 + j) mod n3
+        int cell = m3 + j;
+        if (cell >= n3) cell -= n3;
+        const int slot = j % NS;
+        T *dst = reinterpret_cast<T *>(smem_raw + slot * slot_stride);
+        mbar_expect_tx(&full[slot], (uint32_t)((size_t)lslab * sizeof(T)));
+        const T *src = in + base + (long)cell * slab;
+#pragma unroll
+        for (int l3 = 0; l3 < O; ++l3) {
+            const uint32_t b1 = (uint32_t)((size_t)first_cells * O * N1 * sizeof(T));
+            bulk_g2s(dst + l3 * PR * N1, src + l3 * N2 * N1 + (long)rs * O * N1, b1, &full[slot]);
+            if (first_cells < RC)
+                bulk_g2s(dst + l3 * PR * N1 + (long)first_cells * O * N1, src + l3 * N2 * N1,
+                         (uint32_t)((size_t)(RC - first_cells) * O * N1 * sizeof(T)), &full[slot]);
+        }
+    };
+    if (tid == 0)
+        for (int j = 0; j < NS && j < n3; ++j) issue(j);
+
+    // (k1,k2)-swept values of the thread's two cells: k1 rule on the three source cells, k2 rule twice
+    auto k12_from = [&](const T *sl, T (&wa)[O][O][O], T (&wb)[O][O][O]) {
+#pragma unroll
+        for (int l3 = 0; l3 < O; ++l3) {
+            T tk[3][O][O];
+#pragma unroll
+            for (int e2 = 0; e2 < 3; ++e2)
+#pragma unroll
+                for (int l2 = 0; l2 < O; ++l2) {
+                    T r0[O], r1[O];
+                    load_cell<T, O>(sl + l3 * PR * N1 + offa + (e2 * O + l2) * N1, r0);
+                    load_cell<T, O>(sl + l3 * PR * N1 + offb + (e2 * O + l2) * N1, r1);
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) tk[e2][l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+                }
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a0[O], a1[O], a2[O];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) { a0[l] = tk[0][l][j1]; a1[l] = tk[1][l][j1]; a2[l] = tk[2][l][j1]; }
+                    wa[l3][j2][j1] = chain<T, O>(A2, B2, j2, a0, a1);
+                    wb[l3][j2][j1] = chain<T, O>(A2, B2, j2, a1, a2);
+                }
+        }
+    };
+    auto a_half = [&](const T (&w)[O][O][O], T (&acc)[O][O][O]) {
+#pragma unroll
+        for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2)
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a = mul_t<T>(A3[j3 * O], w[0][j2][j1]);
+#pragma unroll
+                    for (int l = 1; l < O; ++l) a = fma_t<T>(A3[j3 * O + l], w[l][j2][j1], a);
+                    acc[j3][j2][j1] = a;
+                }
+    };
+    auto b_half_put = [&](const T (&acc)[O][O][O], const T (&w)[O][O][O], T *dst) {
+#pragma unroll
+        for (int j3 = 0; j3 < O; ++j3)
+#pragma unroll
+            for (int j2 = 0; j2 < O; ++j2) {
+                T res[O];
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) {
+                    T a = acc[j3][j2][j1];
+#pragma unroll
+                    for (int l = 0; l < O; ++l) a = fma_t<T>(B3[j3 * O + l], w[l][j2][j1], a);
+                    res[j1] = a;
+                }
+                T *p = dst + (long)j3 * N2 * N1 + (long)j2 * N1;
+                if constexpr (O % 2 == 0) {
+                    using V2 = Vec<T, 2>;
+#pragma unroll
+                    for (int j1 = 0; j1 < O; j1 += 2) {
+                        V2 vv; vv.v[0] = res[j1]; vv.v[1] = res[j1 + 1];
+                        *reinterpret_cast<V2 *>(p + j1) = vv;
+                    }
+                } else {
+#pragma unroll
+                    for (int j1 = 0; j1 < O; ++j1) p[j1] = res[j1];
+                }
+            }
+    };
+    auto park_put = [&](int which, const T (&w)[O][O][O]) {
+#pragma unroll
+        for (int a = 0; a < O; ++a)
+#pragma unroll
+            for (int b = 0; b < O; ++b)
+#pragma unroll
+                for (int d = 0; d < O; ++d) park[((which * O3) + (a * O + b) * O + d) * nthr + tid] = w[a][b][d];
+    };
+    auto park_get = [&](int which, T (&w)[O][O][O]) {
+#pragma unroll
+        for (int a = 0; a < O; ++a)
+#pragma unroll
+            for (int b = 0; b < O; ++b)
+#pragma unroll
+                for (int d = 0; d < O; ++d) w[a][b][d] = park[((which * O3) + (a * O + b) * O + d) * nthr + tid];
+    };
+    const long own_a = (long)(c2_0 + t2) * O * N1 + (long)c1 * O;      // first of this thread's two cells in a global slab
+    const long own_b = own_a + (long)O * N1;
+
+    T acca[O][O][O], accb[O][O][O];
+    for (int j = 0; j < n3; ++j) {
+        const int slot = j % NS;
+        mbar_wait(&full[slot], (uint32_t)((j / NS) & 1));
+        T wa[O][O][O], wb[O][O][O];
+        if (active) k12_from(reinterpret_cast<const T *>(smem_raw + slot * slot_stride), wa, wb);
+        __syncthreads();                                     // slab consumed
+        if (tid == 0 && j + NS < n3) issue(j + NS);
+        if (active) {
+            if (j == 0) {
+                park_put(0, wa); park_put(1, wb);
+            } else {
+                T *dst = out + base + (long)(j - 1) * slab;
+                b_half_put(acca, wa, dst + own_a);
+                b_half_put(accb, wb, dst + own_b);
+            }
+            a_half(wa, acca);
+            a_half(wb, accb);
+        }
+    }
+    if (active) {                                            // closes the periodic lines
+        T wf[O][O][O];
+        T *dst = out + base + (long)(n3 - 1) * slab;
+        park_get(0, wf);
+        b_half_put(acca, wf, dst + own_a);
+        park_get(1, wf);
+        b_half_put(accb, wf, dst + own_b);
+    }
+}
+
+}  // namespace sldg

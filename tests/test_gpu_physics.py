@@ -281,6 +281,7 @@ def test_advect_x_twice_is_bitwise_the_group_twice(monkeypatch, shape, parts, dt
     dx, dv, cells, o = shape
     if parts:
         monkeypatch.setenv("SLDG_XTRIPLE_PARTS", parts)
+    monkeypatch.setenv("SLDG_TWICE_TRIPLE", "1")            # the 3+3 D one-pass variant is off by default, tested all the same
     lo = (0.0,) * dx + (-4.0, -3.0, -5.0)[:dv]
     hi = tuple(2 * np.pi * (1 + 0.5 * a) for a in range(dx)) + (4.5, 3.5, 4.0)[:dv]
     cfg = W.Config("x2", dx, dv, cells, o, lo, hi)

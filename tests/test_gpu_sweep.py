@@ -274,10 +274,12 @@ def test_ab_tables_are_rounded_once(oracle, o):
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("amp", [2.5, 0.9])
 @pytest.mark.parametrize("o", [1, 2, 3])
-def test_fused_triple_is_bitwise_the_three_sweeps_3p3(oracle, o, amp, dtype):
+@pytest.mark.parametrize("one", ["0", "1"])
+def test_fused_triple_is_bitwise_the_three_sweeps_3p3(oracle, monkeypatch, o, amp, dtype, one):
     """x_1,x_2,x_3 and v_1,v_2,v_3 in one pass each (o <= 2: the triple kernel; o = 3: pair + single);
     amp = 2.5: the raw v-triple with shifts of a cell or more runs as single sweeps (sldg.h)."""
     import torch
+    monkeypatch.setenv("SLDG_XTRIPLE_ONE", one)           # part-plane x-triple: one / two x_2-cells per thread
     cfg = W.Config("t33", 3, 3, (5, 4, 6, 4, 5, 3), o, (0.0,) * 6, (5.0, 4.0, 6.0, 4.0, 5.0, 3.0))
     rng = np.random.default_rng(31 + o)
     f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
