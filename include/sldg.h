@@ -155,6 +155,8 @@ int sldg_step(sldg_ctx *ctx, double dt);
  * half-steps that end one step and begin the next -- nothing happens between them when no invariant is written
  * -- done as ONE pass over f: x(dt/2) applied twice inside the kernel (sldg_advect_x_twice), not x(dt).
  * Per step: v-group (1R+1W), x-group twice (1R+1W), rho (1R) instead of the 7 N s of sldg_step in d_x >= 2.
+ * Where no kernel applies the whole x-group twice in one pass (d_x = 2 with order >= 4, d_x = 3: there two passes of
+ * the x-triple are faster than its twice-applied variant) the call is nsteps calls of sldg_step.
  * f(t_n) is materialised only at the end; call sldg_diagnostics etc. between calls of sldg_step_n. */
 int sldg_step_n(sldg_ctx *ctx, double dt, int nsteps);
 

@@ -1620,8 +1620,11 @@ extern "C" int sldg_advect_x_twice(sldg_ctx *c, double tau) {
 extern "C" int sldg_step_n(sldg_ctx *c, double dt, int nsteps) {
     if (!c || nsteps < 0) return SLDG_ERR_ARG;
     if (nsteps == 0) return SLDG_OK;
-    // launch-bound problems replay the CUDA graph of one step; merging is for the bandwidth-bound ones
-    if (c->use_graph || nsteps == 1 || !c->tune.twice) {
+    // launch-bound problems replay the CUDA graph of one step; merging is for the bandwidth-bound ones, and only
+    // where one kernel applies the whole x-group twice (else it would be the same passes as sldg_step)
+    const bool one_pass = c->dx == 1 || (c->use_fuse && c->dx == 2 && c->o <= 3) ||
+                          (c->use_fuse && c->dx == 3 && c->o <= 2 && c->tune.twice_triple);
+    if (c->use_graph || nsteps == 1 || !c->tune.twice || !one_pass) {
         for (int s = 0; s < nsteps; ++s) {
             int rc = sldg_step(c, dt);
             if (rc) return rc;

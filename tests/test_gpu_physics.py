@@ -317,6 +317,7 @@ def test_step_n_is_n_steps(oracle, monkeypatch, shape, dtype):
     oracle's n steps within the north-star tolerance."""
     dx, dv, cells, o = shape
     monkeypatch.setenv("SLDG_NO_GRAPH", "1")          # small test shapes would otherwise replay the one-step graph
+    monkeypatch.setenv("SLDG_TWICE_TRIPLE", "1")      # 3+3 D merges only on request (two passes are faster there)
     cfg = W.Config("sn", dx, dv, cells, o, (0.0,) * dx + (-6.0,) * dv, (4 * np.pi,) * dx + (6.0,) * dv, dt=0.1,
                    kind="landau", eps=0.05, k=0.5)
     g = _grid(oracle, cfg)
