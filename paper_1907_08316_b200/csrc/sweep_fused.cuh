@@ -513,7 +513,9 @@ namespace sldg {
 // No raw-value registers and no register prefetch: at o = 3, 4 the register pair kernel is
 // occupancy-starved (168 / 255 registers), this one is not.
 // ------------------------------------------------------------------------------------------
-template <typename T, int O>
+// K1ID: the k1 rule is the identity (A = I, B = 0, offset 0) and is skipped: the kernel is then the single x_2
+// sweep, staged slab by slab by the copy engine (used for sldg_translate / sldg_advect along x_2).
+template <typename T, int O, bool K1ID = false>
 __global__ void __launch_bounds__(256)
 sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2,
                          const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
@@ -530,14 +532,14 @@ sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, 
     const int c1 = tid;
     const bool active = c1 < n1;
 
-    const long q1 = (base / qdiv1) % qmod1, q2 = (base / qdiv2) % qmod2;
+    const long q1 = K1ID ? 0 : (base / qdiv1) % qmod1, q2 = (base / qdiv2) % qmod2;
     T A1[O * O], B1[O * O], A2[O * O], B2[O * O];
 #pragma unroll
     for (int e = 0; e < O * O; ++e) {
-        A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1];
+        if constexpr (!K1ID) { A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1]; }
         A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
     }
-    const int m1 = mtab1[q1], m2 = mtab2[q2];
+    const int m1 = K1ID ? 0 : mtab1[q1], m2 = mtab2[q2];
     int sa1 = (active ? c1 : 0) + m1; if (sa1 >= n1) sa1 -= n1;
     int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
 
@@ -562,9 +564,14 @@ sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, 
         for (int l2 = 0; l2 < O; ++l2) {
             T r0[O], r1[O];
             load_cell<T, O>(sl + l2 * N1 + (long)sa1 * O, r0);
-            load_cell<T, O>(sl + l2 * N1 + (long)sb1 * O, r1);
+            if constexpr (K1ID) {
 #pragma unroll
-            for (int j1 = 0; j1 < O; ++j1) w[l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+                for (int j1 = 0; j1 < O; ++j1) w[l2][j1] = r0[j1];
+            } else {
+                load_cell<T, O>(sl + l2 * N1 + (long)sb1 * O, r1);
+#pragma unroll
+                for (int j1 = 0; j1 < O; ++j1) w[l2][j1] = chain<T, O>(A1, B1, j1, r0, r1);
+            }
         }
     };
     auto emit = [&](int i2, const T (&w0)[O][O], const T (&w1)[O][O]) {
