@@ -636,8 +636,12 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
     } else {
         bool done = false;
         const long Nk = (long)n * O;
-        int W = 512 / (int)sizeof(T);                        // 512-byte rows (64 columns in fp64): +0.5-0.9 % over 256 B at config 4
+        // rows of up to 1 KB (at most 128 columns = one per thread), halved below until the tile fits: 512-byte rows at
+        // configs 3 and 4 (+0.5-0.9 % over 256 B), 1 KB rows at config 5 (40-node lines: v-sweeps 6.35-6.73 -> 6.64-6.85 TB/s)
+        int W = 1024 / (int)sizeof(T);
+        if (W > 128) W = 128;
         if (c->tune.tile_w) W = c->tune.tile_w;              // tuning knob (columns per tile), validated in sldg_create
+        while (W > 8 && W > inner) W /= 2;                   // never wider than the line of columns
         int nbox = (int)cdiv(Nk, 256);
         int box_rows = (int)cdiv(Nk, nbox);
         while (W > 8 && (size_t)nbox * box_rows * W * sizeof(T) > 100 * 1024) W /= 2;
