@@ -1059,8 +1059,29 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
                 (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
             return 0;
         };
+        // two k2-cells per thread (sweep_vtriple_tile2_kernel): threads = W x 4 x C2 / 2, the windows' first cells parked
+        auto launch2 = [&](auto kern, int W, int C2, int NS) -> int {
+            const long blocks = (inner1 / W) * (n1 / 4) * (n2 / C2) * outer3;
+            if (inner1 % W || n2 % C2 || (W * sizeof(T)) % 16 || blocks >= (1L << 31)) return 1;
+            sldg_ctx::TmapSlot &ts = c->tmap5[c->cur];
+            if (!ts.valid || ts.p0 != W) {
+                ts.valid = make_tensor_map_5d(&ts.map, in, sizeof(T) == 8, (uint64_t)inner1, (uint64_t)n1 * O,
+                                              (uint64_t)n2 * O, (uint64_t)n3 * O, (uint64_t)outer3, W, O, O, O);
+                ts.p0 = W;
+            }
+            if (!ts.valid) return 1;
+            const int thr = W * 2 * C2;
+            const size_t smem = (size_t)NS * 6 * (C2 + 2) * O * O * O * W * sizeof(T) + (size_t)2 * O * O * O * thr * sizeof(T);
+            if (smem > 226 * 1024 || ensure_smem(c, kern, smem) != cudaSuccess) { cudaGetLastError(); return 1; }
+            kern<<<(unsigned)blocks, thr, smem, c->stream>>>(
+                ts.map, in, out, inner1, n1, n2, n3, outer3, mm[0], (const T *)ab[0], cnt1, qd[0], qm[0], mm[1],
+                (const T *)ab[1], cnt2, qd[1], qm[1], mm[2], (const T *)ab[2], cnt3, qd[2], qm[2]);
+            return 0;
+        };
         int rc = 1;
         switch (c->tune.vt_variant) {
+        case 12: rc = launch2(sweep_vtriple_tile2_kernel<T, O, 32, 2, 2, 2>, 32, 2, 2); break;
+        case 13: rc = launch2(sweep_vtriple_tile2_kernel<T, O, 32, 4, 2, 1>, 32, 4, 2); break;
         // kept for A/B runs (DESIGN.md section 5 lists what the others measured): 0 = round-1 geometry (one block of
         // 4 x 4 cells), 1 = the same with per-warp slot release and a 3-deep ring, 2 = fp64 default, 10 = fp32 default
         case 0: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 4, 2, 1, false>, 32, 4, 2); break;
@@ -1068,9 +1089,10 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
         case 2: rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 2, 2, false>, 32, 2, 2); break;
         case 10: rc = launch(sweep_vtriple_tile_kernel<T, O, 64, 1, 2, 2, false>, 64, 1, 2); break;
         default:
-            // fp32: 64 columns keep the rows at 256 bytes (9.3 -> 8.5 ms at config 5); fp64: two resident blocks of
-            // 4 x 2 cells (14.8 -> 13.9 ms)
-            if (sizeof(T) == 4) rc = launch(sweep_vtriple_tile_kernel<T, O, 64, 1, 2, 2, false>, 64, 1, 2);
+            // two k2-cells per thread, two resident blocks of 4 x 2 cells: fp64 13.6 -> 12.6 ms at config 5 (32 columns),
+            // fp32 8.35 -> 6.7 ms (64 columns keep the rows at 256 bytes); then the one-cell geometries
+            if constexpr (sizeof(T) == 4) rc = launch2(sweep_vtriple_tile2_kernel<T, O, 64, 2, 2, 2>, 64, 2, 2);
+            if (rc) rc = launch2(sweep_vtriple_tile2_kernel<T, O, 32, 2, 2, 2>, 32, 2, 2);
             if (rc) rc = launch(sweep_vtriple_tile_kernel<T, O, 32, 2, 2, 2, false>, 32, 2, 2);
             break;
         }
