@@ -1392,7 +1392,7 @@ int run_vall_dv(sldg_ctx *c) {
     constexpr int VMAX = 16 / (int)sizeof(T);
     const VSplit g = vsplit<T>(c, 8);
     if (g.small) launch_vall<T, 1, DV, 16, true, 32>(c, g.splits, g.vps);
-    else if (g.vec == VMAX) launch_vall<T, VMAX, DV, 8, false, 128>(c, g.splits, g.vps);
+    else if (g.vec == VMAX) launch_vall<T, VMAX, DV, 16, false, 128>(c, g.splits, g.vps);
     else if (g.vec == 2) launch_vall<T, 2, DV, 8, false, 128>(c, g.splits, g.vps);
     else launch_vall<T, 1, DV, 8, false, 128>(c, g.splits, g.vps);
     LAUNCH_CHECK(c);
