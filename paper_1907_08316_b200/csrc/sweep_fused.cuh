@@ -517,20 +517,27 @@ namespace sldg {
 // sweep, staged slab by slab by the copy engine (used for sldg_translate / sldg_advect along x_2).
 template <typename T, int O, bool K1ID = false>
 __global__ void __launch_bounds__(256)
-sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2,
+sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2, int ppb, long planes,
                          const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
                          const int *__restrict__ mtab2, const T *__restrict__ ab2, long count2, long qdiv2, long qmod2) {
+    // ppb planes per block (> 1 when the x_1 line has fewer cells than a warp has lanes: n_1 = 16 left half of
+    // every warp idle); each plane has its own shifts, its own sub-slot of every ring slot and its own slab order
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     constexpr int NS = 4;                                   // ring depth
+    constexpr int PPB_MAX = 8;
     __shared__ __align__(8) uint64_t full[NS];
     const long N1 = (long)n1 * O;
     const long slab = O * N1;                                // elements per k2-cell of one plane
     const size_t slab_bytes = (size_t)slab * sizeof(T);
-    const size_t slot_stride = (slab_bytes + 127) & ~(size_t)127;
-    const long base = (long)blockIdx.x * n2 * slab;          // planes are contiguous
+    const size_t sub_stride = (slab_bytes + 127) & ~(size_t)127;
+    const size_t slot_stride = sub_stride * ppb;
     const int tid = threadIdx.x;
-    const int c1 = tid;
-    const bool active = c1 < n1;
+    const int pl = tid / n1;                                 // plane of this thread within the block
+    const int c1 = tid - pl * n1;
+    const long plane0 = (long)blockIdx.x * ppb;
+    const bool active = pl < ppb && plane0 + pl < planes;
+    const long base = (active ? plane0 + pl : plane0) * n2 * slab;          // planes are contiguous
+    const size_t sub_off = (size_t)(active ? pl : 0) * sub_stride;
 
     const long q1 = K1ID ? 0 : (base / qdiv1) % qmod1, q2 = (base / qdiv2) % qmod2;
     T A1[O * O], B1[O * O], A2[O * O], B2[O * O];
@@ -548,18 +555,33 @@ sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, 
         for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
     }
     __syncthreads();
-    auto issue = [&](int j) {                                // slab j <-> source k2-cell (m2 + j) mod n2
-        int cell = m2 + j;
-        if (cell >= n2) cell -= n2;
+    // thread 0 issues the copies of every plane of the block: their cell offsets
+    int m2s[PPB_MAX];
+    int nloc = 0;
+    if (tid == 0) {
+        for (int p = 0; p < ppb && p < PPB_MAX; ++p)
+            if (plane0 + p < planes) {
+                m2s[p] = mtab2[(((plane0 + p) * n2 * slab) / qdiv2) % qmod2];
+                nloc = p + 1;
+            }
+    }
+    auto issue = [&](int j) {                                // slab j <-> source k2-cell (m2 + j) mod n2, per plane
         const int slot = j % NS;
-        mbar_expect_tx(&full[slot], (uint32_t)slab_bytes);
-        bulk_g2s(smem_raw + slot * slot_stride, in + base + (long)cell * slab, (uint32_t)slab_bytes, &full[slot]);
+        mbar_expect_tx(&full[slot], (uint32_t)(slab_bytes * nloc));
+#pragma unroll
+        for (int p = 0; p < PPB_MAX; ++p)
+            if (p < nloc) {
+                int cell = m2s[p] + j;
+                if (cell >= n2) cell -= n2;
+                bulk_g2s(smem_raw + slot * slot_stride + p * sub_stride, in + ((plane0 + p) * n2 + cell) * slab,
+                         (uint32_t)slab_bytes, &full[slot]);
+            }
     };
     if (tid == 0)
         for (int j = 0; j < NS && j < n2; ++j) issue(j);
 
     auto k1_from_slab = [&](int slot, T (&w)[O][O]) {       // w[l2][j1]
-        const T *sl = reinterpret_cast<const T *>(smem_raw + slot * slot_stride);
+        const T *sl = reinterpret_cast<const T *>(smem_raw + slot * slot_stride + sub_off);
 #pragma unroll
         for (int l2 = 0; l2 < O; ++l2) {
             T r0[O], r1[O];
