@@ -623,10 +623,16 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
         int ppb = 32 / n1;
         if (ppb < 1) ppb = 1;
         if (ppb > 8) ppb = 8;
-        CUDA_TRY(c, ensure_smem(c, sweep_xpair_plane_kernel<T, O, true>, 4 * slot * ppb));
         const int blk = (int)(cdiv((long)ppb * n1, 32) * 32);
-        sweep_xpair_plane_kernel<T, O, true><<<(unsigned)cdiv(outer, ppb), blk, 4 * slot * ppb, c->stream>>>(
-            in, out, n1, n, ppb, outer, nullptr, nullptr, 0, 1, 1, c->d_m, (const T *)c->d_ab, count, qd2, qm2);
+        if (ppb > 1) {
+            CUDA_TRY(c, ensure_smem(c, sweep_xpair_plane_kernel<T, O, true, true>, 4 * slot * ppb));
+            sweep_xpair_plane_kernel<T, O, true, true><<<(unsigned)cdiv(outer, ppb), blk, 4 * slot * ppb, c->stream>>>(
+                in, out, n1, n, ppb, outer, nullptr, nullptr, 0, 1, 1, c->d_m, (const T *)c->d_ab, count, qd2, qm2);
+        } else {
+            CUDA_TRY(c, ensure_smem(c, sweep_xpair_plane_kernel<T, O, true>, 4 * slot));
+            sweep_xpair_plane_kernel<T, O, true><<<(unsigned)outer, blk, 4 * slot, c->stream>>>(
+                in, out, n1, n, 1, outer, nullptr, nullptr, 0, 1, 1, c->d_m, (const T *)c->d_ab, count, qd2, qm2);
+        }
     } else if (dim < c->dx) {
         const int dep = c->dx + dim;
         long qdiv = 1;
@@ -819,11 +825,18 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
                 if (ppb < 1) ppb = 1;
                 if (ppb > 8) ppb = 8;
                 const size_t smem_pp = 4 * slot * ppb;
-                CUDA_TRY(c, ensure_smem(c, sweep_xpair_plane_kernel<T, O>, smem_pp));
                 const int blk_pp = (int)(cdiv((long)ppb * n1, 32) * 32);
-                sweep_xpair_plane_kernel<T, O><<<(unsigned)cdiv(planes, ppb), blk_pp, smem_pp, c->stream>>>(
-                    in, out, n1, n2, ppb, planes, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2,
-                    (const T *)c->d_ab2, count2, qd2, qm2);
+                if (ppb > 1) {
+                    CUDA_TRY(c, ensure_smem(c, sweep_xpair_plane_kernel<T, O, false, true>, smem_pp));
+                    sweep_xpair_plane_kernel<T, O, false, true><<<(unsigned)cdiv(planes, ppb), blk_pp, smem_pp, c->stream>>>(
+                        in, out, n1, n2, ppb, planes, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2,
+                        (const T *)c->d_ab2, count2, qd2, qm2);
+                } else {
+                    CUDA_TRY(c, ensure_smem(c, sweep_xpair_plane_kernel<T, O>, smem_pp));
+                    sweep_xpair_plane_kernel<T, O><<<(unsigned)planes, blk_pp, smem_pp, c->stream>>>(
+                        in, out, n1, n2, 1, planes, c->d_m, (const T *)c->d_ab, count1, qd1, qm1, c->d_m2,
+                        (const T *)c->d_ab2, count2, qd2, qm2);
+                }
             }
             LAUNCH_CHECK(c);
             c->cur ^= 1;

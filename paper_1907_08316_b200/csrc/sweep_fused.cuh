@@ -515,7 +515,7 @@ namespace sldg {
 // ------------------------------------------------------------------------------------------
 // K1ID: the k1 rule is the identity (A = I, B = 0, offset 0) and is skipped: the kernel is then the single x_2
 // sweep, staged slab by slab by the copy engine (used for sldg_translate / sldg_advect along x_2).
-template <typename T, int O, bool K1ID = false>
+template <typename T, int O, bool K1ID = false, bool MULTI = false>
 __global__ void __launch_bounds__(256)
 sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, int n2, int ppb, long planes,
                          const int *__restrict__ mtab1, const T *__restrict__ ab1, long count1, long qdiv1, long qmod1,
@@ -524,7 +524,8 @@ sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, 
     // every warp idle); each plane has its own shifts, its own sub-slot of every ring slot and its own slab order
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     constexpr int NS = 4;                                   // ring depth
-    constexpr int PPB_MAX = 8;
+    constexpr int PPB_MAX = MULTI ? 8 : 1;
+    if constexpr (!MULTI) ppb = 1;                           // one plane per block: everything below folds to that
     __shared__ __align__(8) uint64_t full[NS];
     const long N1 = (long)n1 * O;
     const long slab = O * N1;                                // elements per k2-cell of one plane
@@ -532,8 +533,8 @@ sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, 
     const size_t sub_stride = (slab_bytes + 127) & ~(size_t)127;
     const size_t slot_stride = sub_stride * ppb;
     const int tid = threadIdx.x;
-    const int pl = tid / n1;                                 // plane of this thread within the block
-    const int c1 = tid - pl * n1;
+    const int pl = MULTI ? tid / n1 : (tid < n1 ? 0 : 1);    // plane of this thread within the block
+    const int c1 = MULTI ? tid - pl * n1 : tid;
     const long plane0 = (long)blockIdx.x * ppb;
     const bool active = pl < ppb && plane0 + pl < planes;
     const long base = (active ? plane0 + pl : plane0) * n2 * slab;          // planes are contiguous
