@@ -610,11 +610,12 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
             sweep_x1_kernel<T, O><<<(unsigned)(ngroups * bpg), block, 0, c->stream>>>(
                 in, out, n, ngroups, cpg, cpb, bpg, c->d_m, (const T *)c->d_ab, count, c->N[c->dx]);
         }
-    } else if (dim == 1 && c->dx >= 2 && c->use_tma && c->tune.plane_single && c->cells[0] <= 256 && n >= 3 &&
+    } else if (dim == 1 && c->dx >= 2 && sizeof(T) == 8 && c->use_tma && c->tune.plane_single && c->cells[0] <= 256 && n >= 3 &&
                ((size_t)O * c->cells[0] * O * sizeof(T)) % 16 == 0 &&
                4 * (((size_t)O * c->cells[0] * O * sizeof(T) + 127) & ~(size_t)127) <= 96 * 1024 && outer < (1L << 31)) {
         // x_2: one block per (x_1,x_2) plane, the plane kernel of the fused x-pair with the x_1 rule skipped (slabs
-        // streamed by the copy engine): config 4 dim 1 6.40 -> 6.7 TB/s against the register-window kernel below
+        // streamed by the copy engine): config 4 dim 1 6.44 -> 6.6 TB/s against the register-window kernel below; fp64
+        // only (fp32, config 4: 5.9 against 6.4 TB/s for the 128-bit register-window kernel)
         const int n1 = c->cells[0];
         const size_t slot = ((size_t)O * n1 * O * sizeof(T) + 127) & ~(size_t)127;
         long qd2 = 1;                                        // q of a plane: (first element / qd2) % qm2
