@@ -547,7 +547,7 @@ sweep_xpair_plane_kernel(const T *__restrict__ in, T *__restrict__ out, int n1, 
         if constexpr (!K1ID) { A1[e] = ab1[(long)e * count1 + q1]; B1[e] = ab1[(long)(O * O + e) * count1 + q1]; }
         A2[e] = ab2[(long)e * count2 + q2]; B2[e] = ab2[(long)(O * O + e) * count2 + q2];
     }
-    const int m1 = K1ID ? 0 : mtab1[q1], m2 = mtab2[q2];
+    const int m1 = K1ID ? 0 : mtab1[q1];                     // (the k2 offsets are needed by thread 0 only, below)
     int sa1 = (active ? c1 : 0) + m1; if (sa1 >= n1) sa1 -= n1;
     int sb1 = sa1 + 1; if (sb1 == n1) sb1 = 0;
 
