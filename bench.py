@@ -536,10 +536,11 @@ def run_ours(args):
                 steps_tab[c2.name] = strang_step_table(torch, Sldg, c2, "f64", nst)
             except Exception as exc:
                 steps_tab[c2.name] = {"error": str(exc)}
-        if args.workload == "config4":          # the paper's section-7 set-ups (1+3 D, 2+3 D at o = 4), context only
-            for c2 in (W.MIXED13, W.MIXED23):
+        if args.workload == "config4":          # the paper's own set-ups, context only: its section-7 mixed dimensions
+            # (1+3 D, 2+3 D at o = 4) and its headline 2+2 D run at o = 4 (60^4 cells, eq. (2); 470 GB/s on a V100)
+            for c2 in (W.MIXED13, W.MIXED23, W.PAPER_TWOSTREAM):
                 try:
-                    steps_tab[c2.name] = strang_step_table(torch, Sldg, c2, "f64", c2.steps)
+                    steps_tab[c2.name] = strang_step_table(torch, Sldg, c2, "f64", min(c2.steps, 5) if c2.steps else 5)
                 except Exception as exc:
                     steps_tab[c2.name] = {"error": str(exc)}
         line["strang_steps_fused"] = steps_tab
