@@ -188,6 +188,41 @@ int sldg_invariants(sldg_ctx *ctx, double *mass, double *l2, double *electric_en
 /* Number of kernels this context has launched since sldg_create (bench "gpu_launches"). */
 unsigned long long sldg_launch_count(const sldg_ctx *ctx);
 
+/* The rho pass (as sldg_compute_rho) for callers that are not allowed to allocate device memory.
+ *
+ * Every context-based call needs sldg_create, and sldg_create calls cudaMalloc for its tables.  Some users
+ * cannot have that: a host code that gave the whole device heap to its own pool at start-up, a plug-in or
+ * callback inside another program's time loop (an allocation may synchronise the whole device and stall that
+ * program's other streams), a job with a memory budget fixed and audited before it starts.  This one call needs
+ * no context and calls no cudaMalloc, cudaFree or any library routine that allocates:
+ *
+ *     rho[x] = - sum_{v < V} Wv[v] * f[v*X + x],   x < X        (fp64 products and sums for both dtypes)
+ *
+ *   f_device    X*V values of type T = dtype in the canonical layout (x fastest); device memory; read only
+ *   Wv_device   V doubles, the quadrature weight of every v-node (prod_a h_a w_j on [0,1]); device; read only
+ *   rho_device  X doubles; device; written
+ *   cuda_stream a cudaStream_t of the CURRENT device (0 = legacy default); the kernels are enqueued on it and
+ *               the call returns without synchronising
+ *   err/err_len optional caller-owned buffer for a message when the call fails (may be NULL / 0)
+ * All three arrays must live on the device that is current in the calling thread.
+ *
+ * The partial sums between its two kernels live in a fixed device array that is part of the library image:
+ * SLDG_RHO_NOALLOC_SCRATCH_BYTES (4 MiB) on every GPU that loads the library, held until the process exits.
+ * Hence the limit: X <= SLDG_RHO_NOALLOC_MAX_X x-nodes (any V); a larger X returns SLDG_ERR_ARG with the
+ * reason in err and launches nothing.  (Config 4 has X = 147 456, config 5 X = 32 768.)
+ *
+ * The FIRST call on each device looks up the array's device address (cudaGetSymbolAddress) and the SM count
+ * before it launches; make that first call outside any stream capture.
+ * All calls on a device share the one array.  Nothing in it has to start at zero -- each call's first kernel
+ * writes every partial sum its second kernel reads, so what an earlier call left behind is never read -- but two
+ * calls whose kernels can overlap on the GPU (different streams, no dependency between them) race on it: keep
+ * calls on one device on one stream, or order them with events.
+ * The result agrees with sldg_compute_rho to rounding (the number of partial sums differs), not bit for bit. */
+#define SLDG_RHO_NOALLOC_SCRATCH_BYTES 4194304
+#define SLDG_RHO_NOALLOC_MAX_X 524288
+int sldg_rho_noalloc(const void *f_device, sldg_dtype dtype, size_t X, size_t V, const double *Wv_device,
+                     double *rho_device, void *cuda_stream, char *err, size_t err_len);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,6 +19,7 @@ EXPORTS = [
     "sldg_node_coords", "sldg_set_initial", "sldg_get_f", "sldg_current", "sldg_fill_uniform",
     "sldg_translate", "sldg_translate_dev", "sldg_advect", "sldg_advect_pair", "sldg_translate_pair_dev", "sldg_advect_triple", "sldg_translate_triple_dev", "sldg_compute_rho", "sldg_poisson_E",
     "sldg_set_E", "sldg_advect_x_rho", "sldg_advect_x_twice", "sldg_step", "sldg_step_n", "sldg_diagnostics", "sldg_moments", "sldg_invariants", "sldg_launch_count",
+    "sldg_rho_noalloc",
 ]
 
 
@@ -62,6 +63,7 @@ def _load():
     lib.sldg_invariants.argtypes = [vp, dp, dp, dp, dp, dp]
     lib.sldg_launch_count.argtypes = [vp]
     lib.sldg_launch_count.restype = C.c_ulonglong
+    lib.sldg_rho_noalloc.argtypes = [vp, C.c_int, C.c_size_t, C.c_size_t, vp, vp, vp, C.c_char_p, C.c_size_t]
     return lib
 
 
@@ -70,6 +72,30 @@ _lib = _load()
 
 class SldgError(RuntimeError):
     pass
+
+
+def rho_noalloc(f, X, V, Wv, rho, stream=None):
+    """sldg_rho_noalloc: rho[x] = -sum_v Wv[v] f[v*X + x] with no device allocation inside the library.
+
+    For callers that may not call cudaMalloc (a host code whose pool owns the whole device heap, a callback in
+    another program's time loop, a fixed memory budget): there is no context, the caller brings every buffer --
+    f (X*V values, float64 or float32), Wv (V float64) and rho (X float64, written), all CUDA tensors on the
+    current device -- and the partial sums sit in a fixed 4 MiB array inside libsldg.so.  X may not exceed
+    SLDG_RHO_NOALLOC_MAX_X (524288).  Calls on one device share that array: keep them on one stream.  The first
+    call on a device also looks the array up; make it outside any stream capture.  Marshalling only."""
+    import torch
+    assert f.is_cuda and Wv.is_cuda and rho.is_cuda and f.is_contiguous() and Wv.is_contiguous() and rho.is_contiguous()
+    assert Wv.dtype == torch.float64 and rho.dtype == torch.float64 and f.dtype in (torch.float64, torch.float32)
+    assert f.numel() == X * V and Wv.numel() == V and rho.numel() == X
+    if stream is None:
+        stream = torch.cuda.current_stream(f.device)
+    err = C.create_string_buffer(512)
+    with torch.cuda.device(f.device):
+        rc = _lib.sldg_rho_noalloc(f.data_ptr(), SLDG_F64 if f.dtype == torch.float64 else SLDG_F32, int(X), int(V),
+                                   Wv.data_ptr(), rho.data_ptr(), stream.cuda_stream, err, len(err))
+    if rc != 0:
+        raise SldgError("sldg_rho_noalloc failed (%d): %s" % (rc, err.value.decode()))
+    return rho
 
 
 class Sldg:
