@@ -83,7 +83,11 @@ int sldg_node_coords(const sldg_ctx *ctx, int dim, double *host_out);
  * cudaMemcpyAsync on the stream followed by a stream synchronise. */
 int sldg_set_initial(sldg_ctx *ctx, const void *f_src, int is_device);
 int sldg_get_f(sldg_ctx *ctx, void *dst, int is_device);
-void *sldg_current(sldg_ctx *ctx);                  /* device pointer holding f now        */
+/* Device pointer holding f now.  The pointer is writable: the library assumes the caller may edit f through
+ * it and forgets the invariants it remembered for the current f (see sldg_invariants).  rho and E held in the
+ * context are NOT dropped; after editing f in place call sldg_compute_rho / sldg_poisson_E (or sldg_diagnostics,
+ * which does both) before a v-sweep that should see the new field. */
+void *sldg_current(sldg_ctx *ctx);
 
 /* Fill the current buffer with f[g] = U(seed, tag, g) in [0,1) rounded to T, g = canonical
  * linear index: the counter-based generator of the config-4 microbenchmark (DESIGN.md
@@ -110,11 +114,14 @@ int sldg_advect(sldg_ctx *ctx, int dim, double dt);
  * calls), but f is read and written once instead of twice.  dim1 < dim2, both x-dimensions or both
  * v-dimensions (their shifts do not depend on each other's coordinate, D:R8).  sldg_step uses this
  * for (x_1,x_2) and (v_1,v_2) unless SLDG_NO_FUSE=1 is set in the environment at sldg_create.
- * The fused v-kernels are built for the physical regime |shift| < 1 cell.  sldg_translate_pair_dev /
- * _triple_dev along v-dimensions therefore assemble the tables first, read back (stream synchronisation)
- * whether any line is shifted by a cell or more, and run such a call as single sweeps -- same result, two
- * (three) passes.  sldg_advect_pair / _triple do not check: a field with |E| dt >= h_v is outside the
- * regime the splitting is accurate in and costs bandwidth there, never correctness. */
+ * The fused v-kernels are built for the physical regime |shift| < 1 cell; a block that meets a line shifted by
+ * a cell or more falls back to reading its neighbours from global memory -- same bits, about 2.5x the time of
+ * the two single sweeps when most lines are that wide.  All four calls are asynchronous like the rest of the
+ * library and none checks the width: a field with |E| dt >= h_v is outside the regime the splitting is accurate
+ * in and costs bandwidth there, never correctness.  A caller that feeds sldg_translate_pair_dev / _triple_dev
+ * wide v-shifts on purpose can set SLDG_ROUTE_WIDE=1 in the environment at sldg_create: those two calls then
+ * assemble the tables first, read back (STREAM SYNCHRONISATION, so not inside a stream capture) whether any
+ * line is a cell or more wide, and run such a call as single sweeps. */
 int sldg_advect_pair(sldg_ctx *ctx, int dim1, int dim2, double dt);
 int sldg_translate_pair_dev(sldg_ctx *ctx, int dim1, const double *shift1_device, size_t count1,
                             int dim2, const double *shift2_device, size_t count2);
@@ -135,7 +142,8 @@ int sldg_compute_rho(sldg_ctx *ctx, double *rho_device_or_null);
  * spectral with the modes |m_a| <= floor((n_a - 1)/2) and the mean mode dropped (D:R6, D:R13). */
 int sldg_poisson_E(sldg_ctx *ctx, double *E_device_or_null);
 
-/* Overwrite the stored E ([dx][X] fp64, host or device): lets a caller drive sldg_advect in v. */
+/* Overwrite the stored E ([dx][X] fp64, host or device): lets a caller drive sldg_advect in v.  The next
+ * sldg_diagnostics / sldg_invariants re-reads f and replaces this E by the one that belongs to the current f. */
 int sldg_set_E(sldg_ctx *ctx, const double *E, int is_device);
 
 /* S:8(f) NEXT-1: the x half-step and the density that follows it ("advection x", "compute rho") as ONE
@@ -143,15 +151,22 @@ int sldg_set_E(sldg_ctx *ctx, const double *E, int is_device);
  * bit-identical), and leaves rho of the result in the context (and in rho_device_or_null, X doubles on the
  * device, if not NULL).  When d_x = 2 or 3 and the fused sweep kernels apply, rho is accumulated while the
  * last sweep writes f (no separate read of f); otherwise it is the sweeps followed by sldg_compute_rho.
- * sldg_step uses this call for its first x half-step. */
+ * sldg_step uses this call for its first x half-step.
+ * Reproducibility: every sum in the library has a fixed order, so a run repeats bit for bit on the same GPU
+ * model and library build.  The NUMBER of partial rows of the rho accumulated here is sized to one wave of
+ * blocks (SM count x resident blocks), and the stand-alone pass sizes its v-splits from the SM count too, so rho
+ * -- and through E every later f -- may differ at rounding level (1e-16 relative per step) between GPU models
+ * or toolkit versions.  f from the sweeps alone (sldg_translate*, sldg_advect* with a given E) has no such
+ * dependence. */
 int sldg_advect_x_rho(sldg_ctx *ctx, double tau, double *rho_device_or_null);
 
 /* Strang step (D:O6 row a-5): x_1..x_dx with dt/2, rho, Poisson, v_1..v_dx with dt,
  * x_1..x_dx with dt/2. */
 int sldg_step(sldg_ctx *ctx, double dt);
 
-/* nsteps Strang steps, bit for bit the result of nsteps calls of sldg_step (up to the rounding-level difference
- * between rho accumulated inside a sweep and rho from its own pass, see sldg_advect_x_rho), with the x
+/* nsteps Strang steps: the result of nsteps calls of sldg_step -- bit for bit when rho is a pass of its own in
+ * both (SLDG_NO_FUSE_RHO=1), else up to the rounding-level difference between rho accumulated inside a sweep
+ * (sldg_step, see sldg_advect_x_rho) and rho from its own pass (this call) -- with the x
  * half-steps that end one step and begin the next -- nothing happens between them when no invariant is written
  * -- done as ONE pass over f: x(dt/2) applied twice inside the kernel (sldg_advect_x_twice), not x(dt).
  * Per step: v-group (1R+1W), x-group twice (1R+1W), rho (1R) instead of the 7 N s of sldg_step in d_x >= 2.
@@ -181,7 +196,11 @@ int sldg_moments(sldg_ctx *ctx, double *momentum, double *kinetic_energy);
  * rho also forms sum W f^2, sum v_a W f and sum |v|^2 W f (S:8(f) NEXT-4 "fused into the rho pass").
  * Outputs as in sldg_diagnostics / sldg_moments (host pointers, any may be NULL; momentum has dv entries);
  * synchronises the stream once.  The library remembers the result until f changes: sldg_diagnostics,
- * sldg_moments and sldg_invariants called in any order on the same f read it from HBM once. */
+ * sldg_moments and sldg_invariants called in any order on the same f read it from HBM once.  "Changes" means:
+ * through a library call (a sweep, a step, sldg_set_initial, sldg_fill_uniform), or possibly through the caller's
+ * own hands -- sldg_current() hands out a writable pointer and therefore forgets the remembered result, and so
+ * does sldg_set_E (the remembered electric energy belonged to the old E).  A caller that keeps a pointer from an
+ * earlier sldg_current() and edits f later must call sldg_current() again before asking for invariants. */
 int sldg_invariants(sldg_ctx *ctx, double *mass, double *l2, double *electric_energy, double *momentum,
                     double *kinetic_energy);
 

@@ -10,7 +10,9 @@
 #include <stdlib.h>
 #include <string.h>
 
-#include <unordered_map>
+#include <map>
+#include <mutex>
+#include <utility>
 #include <vector>
 
 #include "fill.cuh"
@@ -41,9 +43,6 @@ struct sldg_ctx {
     cudaStream_t stream = nullptr;
     int device = 0;                    // the device the context was created on; every entry point runs there
     int sm_count = 148;
-    // dynamic shared memory opt-in (cudaFuncAttributeMaxDynamicSharedMemorySize) is per device and per
-    // kernel: remembered per CONTEXT (a context lives on one device), never in process-wide statics
-    std::unordered_map<const void *, size_t> smem_attr;
     // tuning switches, read from the environment ONCE in sldg_create
     struct Tune {
         int tile_w = 0;                // SLDG_TILE_W: columns per TMA tile of the v-sweeps (0 = default)
@@ -57,6 +56,7 @@ struct sldg_ctx {
         bool twice_triple = false;     // SLDG_TWICE_TRIPLE=1: sldg_step_n also merges the x half-steps in 3+3 D (slower, section 9)
         bool twice = true;             // SLDG_NO_TWICE=1 -> false: sldg_step_n never merges the x half-steps of two steps
         bool fuse_rho = true;          // SLDG_NO_FUSE_RHO=1 -> false: rho is a pass of its own after the x-group
+        bool route_wide = false;       // SLDG_ROUTE_WIDE=1: raw fused v-calls read a flag back (stream sync) and run wide shifts as single sweeps
         bool rho_triple = false;       // SLDG_RHO_TRIPLE=1: also fuse rho into the x-triple (3+3 D: measured break-even, off)
         int x1_chunk_kb = 0, x1_block = 128;   // SLDG_X1_CHUNK_KB / SLDG_X1_BLOCK: bulk x_1 kernel geometry (0 = default)
         int rho_cells = 0;             // SLDG_RHO_CELLS: cells per block range in the fused x-group + rho kernels (0 = default)
@@ -174,11 +174,17 @@ struct DeviceGuard {
     ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
 };
 
-// opt in to `bytes` of dynamic shared memory for `kernel` on this context's device (once per size)
+// Opt in to `bytes` of dynamic shared memory for `kernel` on this context's device.  The attribute
+// (cudaFuncAttributeMaxDynamicSharedMemorySize) belongs to the (device, kernel) pair, not to a context, and
+// cudaFuncSetAttribute stores exactly the value it is given -- so it is remembered process-wide under that key
+// and only ever RAISED: a second context with a smaller grid must not lower what a live context's launches need.
+std::mutex g_smem_mutex;
+std::map<std::pair<int, const void *>, size_t> g_smem_attr;
 template <typename K>
 cudaError_t ensure_smem(sldg_ctx *c, K kernel, size_t bytes) {
     if (bytes <= 32 * 1024) return cudaSuccess;          // static + dynamic must stay under the 48 KB default
-    size_t &have = c->smem_attr[(const void *)kernel];
+    std::lock_guard<std::mutex> lock(g_smem_mutex);
+    size_t &have = g_smem_attr[std::make_pair(c->device, (const void *)kernel)];
     if (bytes <= have) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
     if (e == cudaSuccess) have = bytes;
@@ -228,7 +234,13 @@ extern "C" const char *sldg_last_error(const sldg_ctx *ctx) { return ctx ? ctx->
 extern "C" size_t sldg_num_dofs(const sldg_ctx *ctx) { return ctx ? (size_t)ctx->ndof : 0; }
 extern "C" size_t sldg_num_x(const sldg_ctx *ctx) { return ctx ? (size_t)ctx->X : 0; }
 extern "C" unsigned long long sldg_launch_count(const sldg_ctx *ctx) { return ctx ? ctx->launches : 0; }
-extern "C" void *sldg_current(sldg_ctx *ctx) { return ctx ? ctx->buf[ctx->cur] : nullptr; }
+// The pointer is writable and the buffer is the caller's: whoever asks for it may edit f in place (a source or
+// collision term, a rescale), so the remembered invariants of "the current f" are dropped here.
+extern "C" void *sldg_current(sldg_ctx *ctx) {
+    if (!ctx) return nullptr;
+    ctx->have_inv = false;
+    return ctx->buf[ctx->cur];
+}
 
 extern "C" int sldg_node_coords(const sldg_ctx *ctx, int dim, double *host_out) {
     if (!ctx || !host_out || dim < 0 || dim >= ctx->D) return SLDG_ERR_ARG;
@@ -292,6 +304,7 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
         c->tune.twice_triple = env_flag("SLDG_TWICE_TRIPLE");
         c->tune.xt_parts = env_int("SLDG_XTRIPLE_PARTS", 0, 1, 8);
         c->tune.rho_triple = env_flag("SLDG_RHO_TRIPLE");
+        c->tune.route_wide = env_flag("SLDG_ROUTE_WIDE");
         c->tune.rho_cells = env_int("SLDG_RHO_CELLS", 0, 1, 8);
         c->tune.x1_chunk_kb = env_int("SLDG_X1_CHUNK_KB", 0, 2, 96);
         c->tune.x1_block = env_int("SLDG_X1_BLOCK", 128, 64, 256) / 32 * 32;
@@ -1313,7 +1326,10 @@ extern "C" int sldg_translate_pair_dev(sldg_ctx *c, int dim1, const double *shif
     use_tab(c, 2, c->gen[1], false);
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift1, count1 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma2, shift2, count2 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
-    if (dim1 >= c->dx) {                 // v-pair: wide shifts run as two single sweeps
+    // v-pair: asynchronous by default (a line shifted by a cell or more takes the fused kernel's per-block
+    // fallback: same bits, more traffic); with SLDG_ROUTE_WIDE=1 the call reads back whether any line is that
+    // wide (stream synchronisation) and runs such a call as two single sweeps
+    if (dim1 >= c->dx && c->tune.route_wide) {
         const int dims[2] = {dim1, dim2};
         const size_t counts[2] = {count1, count2};
         bool wide = false;
@@ -1536,6 +1552,7 @@ extern "C" int sldg_set_E(sldg_ctx *c, const double *E, int is_device) {
                                 is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
     if (!is_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     c->have_E = true;
+    c->have_inv = false;               // the remembered electric energy belonged to the E just overwritten
     return SLDG_OK;
 }
 
@@ -1575,7 +1592,7 @@ extern "C" int sldg_translate_triple_dev(sldg_ctx *c, int dim1, const double *sh
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma, shift1, count1 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma2, shift2, count2 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_sigma3, shift3, count3 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
-    if (dim1 >= c->dx) {                 // v-triple: wide shifts run as three single sweeps
+    if (dim1 >= c->dx && c->tune.route_wide) {   // v-triple: as the v-pair (three single sweeps when wide)
         const int dims[3] = {dim1, dim2, dim3};
         const size_t counts[3] = {count1, count2, count3};
         bool wide = false;

@@ -157,10 +157,13 @@ def test_tma_and_plain_kernels_agree_bit_for_bit(monkeypatch):
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("amp", [3.5, 0.9])
 @pytest.mark.parametrize("o", [1, 2, 3, 4])
-def test_fused_pair_is_bitwise_the_two_sweeps_2p2(oracle, o, amp, dtype):
-    """amp = 0.9: |shift| < 1 cell, the regime of the fused v-kernels; amp = 3.5: a raw v-pair with wider
-    shifts is routed to two single sweeps (sldg.h), an x-pair stays one kernel whatever the shift."""
+@pytest.mark.parametrize("route", ["0", "1"])
+def test_fused_pair_is_bitwise_the_two_sweeps_2p2(oracle, monkeypatch, o, amp, dtype, route):
+    """amp = 0.9: |shift| < 1 cell, the regime of the fused v-kernels; amp = 3.5: a raw v-pair with wider shifts
+    stays one (asynchronous) kernel whose blocks take the global-read fallback, or, with SLDG_ROUTE_WIDE=1, is
+    routed to two single sweeps after a flag read-back (sldg.h); an x-pair is one kernel whatever the shift."""
     import torch
+    monkeypatch.setenv("SLDG_ROUTE_WIDE", route)
     cfg = W.Config("p22", 2, 2, (11, 7, 9, 6), o, (0.0,) * 4, (11.0, 7.0, 9.0, 6.0))
     rng = np.random.default_rng(77 + o)
     f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
@@ -173,7 +176,7 @@ def test_fused_pair_is_bitwise_the_two_sweeps_2p2(oracle, o, amp, dtype):
         a.set_initial(f0)
         l0 = a.launch_count()
         a.translate_pair(k1, torch.from_numpy(sig[0]).cuda(), k2, torch.from_numpy(sig[1]).cuda())
-        assert a.launch_count() - l0 == (4 if (k1 >= 2 and amp > 1.0) else 3)     # 2 table kernels + 1 or 2 sweeps
+        assert a.launch_count() - l0 == (4 if (k1 >= 2 and amp > 1.0 and route == "1") else 3)   # 2 table kernels + 1 or 2 sweeps
         fused = a.get_f()
         a.close()
         b = make_solver(cfg, dtype)
@@ -277,9 +280,11 @@ def test_ab_tables_are_rounded_once(oracle, o):
 @pytest.mark.parametrize("one", ["0", "1"])
 def test_fused_triple_is_bitwise_the_three_sweeps_3p3(oracle, monkeypatch, o, amp, dtype, one):
     """x_1,x_2,x_3 and v_1,v_2,v_3 in one pass each (o <= 2: the triple kernel; o = 3: pair + single);
-    amp = 2.5: the raw v-triple with shifts of a cell or more runs as single sweeps (sldg.h)."""
+    amp = 2.5: the raw v-triple with shifts of a cell or more takes the fused kernel's per-block fallback
+    (one = "0") or, with SLDG_ROUTE_WIDE=1 (one = "1"), runs as single sweeps (sldg.h)."""
     import torch
     monkeypatch.setenv("SLDG_XTRIPLE_ONE", one)           # part-plane x-triple: one / two x_2-cells per thread
+    monkeypatch.setenv("SLDG_ROUTE_WIDE", one)            # both settings of the wide-shift routing ride along
     cfg = W.Config("t33", 3, 3, (5, 4, 6, 4, 5, 3), o, (0.0,) * 6, (5.0, 4.0, 6.0, 4.0, 5.0, 3.0))
     rng = np.random.default_rng(31 + o)
     f0 = rng.uniform(0.0, 1.0, cfg.ndof).astype(NPDT[dtype])
@@ -473,3 +478,50 @@ def test_tile_staged_v_triple(oracle, o, dtype, kind):
     a.close(); b.close()
     assert np.array_equal(fused, seq)
     assert rel_err(fused, ref) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("o", [2, 3, 4])
+def test_two_live_contexts_of_different_size_interleaved(o, dtype):
+    """The dynamic shared-memory opt-in belongs to (device, kernel), not to a context, and setting it stores the
+    exact value: a second, smaller context that uses the same kernels must not lower what the first one's launches
+    need.  Two live contexts of the same dtype and order, a large and a small grid, take turns through
+    single sweeps, fused pairs and Strang steps; the large one must come out bit for bit as when it runs alone."""
+    import torch
+    big = W.Config("big", 2, 2, (40, 36, 24, 20), o, (0.0, 0.0, -4.0, -4.0), (4 * np.pi, 4 * np.pi, 4.0, 4.0))
+    small = W.Config("small", 2, 2, (5, 4, 4, 3), o, (0.0, 0.0, -4.0, -4.0), (4 * np.pi, 4 * np.pi, 4.0, 4.0))
+    rng = np.random.default_rng(77)
+    fb = rng.uniform(0.0, 1.0, big.ndof).astype(NPDT[dtype])
+    fs = rng.uniform(0.0, 1.0, small.ndof).astype(NPDT[dtype])
+
+    def shifts(cfg, seed):
+        r = np.random.default_rng(seed)
+        return [r.uniform(-0.4, 0.4, cfg.N[cfg.dx + d] if d < cfg.dx else cfg.X) for d in range(4)]
+
+    def work(s, cfg, seed):
+        sig = shifts(cfg, seed)
+        for d in range(4):
+            s.translate(d, sig[d])
+        dev = [torch.from_numpy(x).cuda() for x in sig]
+        s.translate_pair(0, dev[0], 1, dev[1])
+        s.translate_pair(2, dev[2], 3, dev[3])
+        s.step(0.05)
+
+    alone = make_solver(big, dtype)
+    alone.set_initial(fb)
+    work(alone, big, 1)
+    work(alone, big, 2)
+    want = alone.get_f()
+    alone.close()
+
+    a, b = make_solver(big, dtype), make_solver(small, dtype)
+    a.set_initial(fb)
+    b.set_initial(fs)
+    work(a, big, 1)
+    work(b, small, 3)          # same kernels, smaller shared-memory requests
+    work(a, big, 2)            # failed with "invalid value" when the opt-in was remembered per context
+    work(b, small, 4)
+    got = a.get_f()
+    a.close(); b.close()
+    assert np.all(np.isfinite(got))
+    assert np.array_equal(got, want)
