@@ -12,6 +12,7 @@
  */
 #include "sldg_oracle.h"
 
+#include <float.h>
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
@@ -20,6 +21,14 @@
 #endif
 
 static const double ORACLE_PI = 3.14159265358979323846264338327950288;
+
+/* Guard, not arithmetic: the rule, the A,B quadrature and the rho / mass / l2 / moment sums are "computed in
+ * long double and rounded once" (D:O4, D:O7, D:R12), and the pins hold them to 1e-13.  That needs a long double
+ * with at least the 64-bit mantissa of x87 extended precision.  Where long double is plain double (MSVC, some
+ * ARM ABIs) the sums would silently fall back to the running double sum that the comment above oracle_rho
+ * measures as not good enough; refuse to build there instead.  (binary128 long double, e.g. aarch64 Linux,
+ * passes: slower, at least as accurate.) */
+_Static_assert(LDBL_MANT_DIG >= 64, "the oracle needs long double with >= 64 mantissa bits (x87 extended or wider)");
 
 int oracle_num_threads(void) {
 #ifdef _OPENMP
