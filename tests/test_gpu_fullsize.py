@@ -267,3 +267,23 @@ def test_config4_fp32_full_size_fused_pairs_equal_single_sweeps():
 
 def test_config3_full_size_fused_pairs_equal_single_sweeps():
     _fused_vs_single_fullsize(W.CONFIG3, "f64", [(0, 1), (2, 3)], _smooth_shifts(W.CONFIG3), 10)
+
+
+def test_paper_twostream_validation_run_at_the_papers_size():
+    """S:8(f) NEXT-2 at the paper's own size (section 8 eq. (2)): 2+2 D two-stream, 60^4 cells,
+    o = 4, t <= 100, single against double precision.  The paper: "the difference in the distribution function
+    (infinity norm), the electric field (infinity norm), and the relative difference in electric energy are below
+    2e-4" (P:235).  3.3e9 DOF in fp64 and fp32 side by side (80 GB), 1000 Strang steps each, about a minute."""
+    import torch
+    from paper_1907_08316_b200.examples.two_stream_2p2 import run
+    _need_gb(90)
+    out, trace = run(cells=60, t_end=100.0, dt=0.1, sample_every=10)
+    torch.cuda.empty_cache()
+    assert out["config"]["ndof"] == (60 * 4) ** 4
+    assert out["ee_growth"] > 1e4                         # the instability has developed and saturated
+    assert out["max_df_inf"] < 2e-4                       # the paper's three differences
+    assert out["max_dE_inf"] < 2e-4
+    assert out["max_rel_ee_diff_pointwise"] < 2e-4
+    assert out["max_df_inf_rel_to_fmax"] < 2e-4           # also relative to max f (1.65e-4 measured: the tight one)
+    assert out["mass_drift64"] < 1e-12 and out["mass_drift32"] < 1e-5
+    assert out["energy_drift64"] < 1e-3

@@ -53,7 +53,7 @@ def test_rho_poisson_diagnostics(oracle, shape, dtype):
     mr, l2r, eer = g.diagnostics(f0)
     assert abs(m - mr) <= 1e-13 * abs(mr)
     assert abs(l2 - l2r) <= 1e-13 * abs(l2r)
-    assert abs(ee - eer) <= 1e-11 * abs(eer)
+    assert abs(ee - eer) <= 1e-12 * abs(eer)          # north_star: the ee trace to the bound of f (D:R11 form, one point)
     s.close()
 
 
@@ -189,7 +189,7 @@ def test_invariants_one_read_of_f(oracle, shape, dtype):
     mr, l2r, eer = g.diagnostics(f0)
     Pr, Kr = g.moments(f0)
     assert abs(m - mr) <= 1e-13 * abs(mr) and abs(l2 - l2r) <= 1e-13 * abs(l2r)
-    assert abs(ee - eer) <= 1e-11 * abs(eer)
+    assert abs(ee - eer) <= 1e-12 * abs(eer)          # north_star: the ee trace to the bound of f (D:R11 form, one point)
     assert np.max(np.abs(P - Pr)) <= 1e-13 * np.max(np.abs(Pr)) + 1e-13 * abs(Kr)
     assert abs(K - Kr) <= 1e-13 * abs(Kr)
     # the same f again, through the two older calls: no kernel is launched, same numbers
@@ -371,7 +371,7 @@ def test_mixed_dimension_steps(oracle, shape, dtype):
     cfg = W.Config("mix", dx, dv, cells, 2, lo, hi, dt=0.1, steps=4, kind="landau", eps=0.05, k=0.5)
     got, ref, tg, tr = _run_config(oracle, cfg, dtype, cfg.steps)
     assert rel_err(got, ref) <= TOL[dtype]
-    _check_traces(tg, tr, max(TOL[dtype], 1e-11))
+    _check_traces(tg, tr, TOL[dtype])
 
 
 @pytest.mark.parametrize("o", [4, 5, 6])
@@ -381,7 +381,7 @@ def test_high_order_2p2_steps(oracle, o):
                    dt=0.1, steps=3, kind="landau", eps=0.05, k=0.5)
     got, ref, tg, tr = _run_config(oracle, cfg, "f64", cfg.steps)
     assert rel_err(got, ref) <= TOL["f64"]
-    _check_traces(tg, tr, 1e-11)
+    _check_traces(tg, tr, TOL["f64"])
 
 
 # ---------------------------------------------------------------- NEXT-2: the paper's validation run (eq. (2))
@@ -390,7 +390,7 @@ def test_paper_twostream_parity_small(oracle):
     cfg = W.PAPER_TWOSTREAM.scaled((8, 8, 10, 10), steps=5)
     got, ref, tg, tr = _run_config(oracle, cfg, "f64", cfg.steps)
     assert rel_err(got, ref) <= TOL["f64"]
-    _check_traces(tg, tr, 1e-11)
+    _check_traces(tg, tr, TOL["f64"])
 
 
 def test_paper_twostream_fp32_vs_fp64_reduced():
