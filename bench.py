@@ -27,12 +27,24 @@ sys.path.insert(0, ROOT)
 
 from paper_1907_08316_b200 import workloads as W  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the sweep kernel of each direction, from one
-# ncu capture of this very command at full size (profiles/traffic_launches_r2.md); None where not captured.
-TRAFFIC_BYTES = {
-    ("config4-sweep-2+2", "f64"): {0: 43.497e9 + 43.436e9, 1: 43.829e9 + 43.445e9,
-                                   2: 43.520e9 + 43.432e9, 3: 43.520e9 + 43.433e9},
-}
+TRAFFIC_TABLE = os.path.join(ROOT, "profiles", "traffic_launches_r3.md")
+
+
+def traffic_bytes(workload, dtype):
+    """{dim: dram__bytes_read.sum + dram__bytes_write.sum per launch} of the sweep kernel of each direction, parsed
+    from the table of the ncu capture of this very command at full size (profiles/traffic_launches_r3.md: rows
+    `| <workload> | <dtype> | dim<k> | kernel | read GB | write GB | ...`); {} where nothing was captured."""
+    out = {}
+    try:
+        with open(TRAFFIC_TABLE) as fh:
+            for row in fh:
+                cells = [c.strip() for c in row.strip().strip("|").split("|")]
+                if len(cells) >= 6 and cells[0] == workload and cells[1] == dtype and cells[2].startswith("dim"):
+                    out[int(cells[2][3:])] = (float(cells[4]) + float(cells[5])) * 1e9
+    except (OSError, ValueError):
+        return {}
+    return out
+
 
 METRIC = "achieved_hbm_gbs_per_translation_sweep"
 UNIT = "GB/s"
@@ -447,8 +459,8 @@ def run_ours(args):
     dom = max(dim_avg, key=dim_avg.get)
     roofline = {"bound": "hbm", "achieved": sweep_bytes / dim_avg[dom] / 1e6, "peak": peak, "unit": "GB/s",
                 "frac": sweep_bytes / dim_avg[dom] / 1e6 / peak,
-                "traffic": TRAFFIC_BYTES.get((cfg.name, dtype), {}).get(dom),
-                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/traffic_launches_r2.md",
+                "traffic": traffic_bytes(cfg.name, dtype).get(dom),
+                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, parsed from profiles/traffic_launches_r3.md",
                 "kernel": "translation sweep along dim %d (slowest direction)" % dom,
                 "algorithmic_bytes_per_launch": sweep_bytes, "peak_source": peak_src,
                 "per_direction_gbs": {"dim%d" % d: sweep_bytes / t / 1e6 for d, t in dim_avg.items()},
@@ -528,6 +540,20 @@ def run_ours(args):
                 s2.close(); del s2; torch.cuda.empty_cache()
             except Exception as exc:        # report, never hide
                 extras["%s-%s" % (c2.name, dt_)] = {"error": str(exc)}
+        if args.workload == "config4":
+            # the paper's order axis (Fig. 2: bandwidth at o = 2, 4, 6): single sweeps of the 2+2 D two-stream
+            # set-up at o = 4, 5, 6 on 3.3e9 DOF each (60^4, 48^4, 40^4 cells), physics-like shifts
+            for o_, n_ in ((4, 60), (5, 48), (6, 40)):
+                base = W.PAPER_TWOSTREAM
+                c2 = W.Config("order-axis-2+2-o%d" % o_, 2, 2, (n_,) * 4, o_, base.lo, base.hi, dt=base.dt,
+                              kind=base.kind, eps=base.eps, k=base.k, extra=dict(base.extra))
+                try:
+                    s2 = Sldg.from_config(c2, dtype="f64")
+                    s2.fill_uniform(W.SEED, W.TAG_F)
+                    extras["%s-f64" % c2.name] = sweep_table(torch, s2, c2, "f64", reps=10, warm=3)
+                    s2.close(); del s2; torch.cuda.empty_cache()
+                except Exception as exc:
+                    extras["%s-f64" % c2.name] = {"error": str(exc)}
         line["sweeps_other_configs"] = extras
         steps_tab = {}
         for name, nst in (("config3", 20), ("config5", 5)):

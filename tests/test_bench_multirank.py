@@ -77,3 +77,14 @@ def test_reference_arm_json_contract():
     assert d["impl"] == "reference" and d["unit"] == "GB/s" and d["value"] > 0 and d["vs_baseline"] is None
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and "workload" in d["config"]
+
+
+def test_roofline_traffic_is_parsed_from_the_profile_table():
+    """bench.py carries no typed-in DRAM byte counts: roofline.traffic comes from the ncu table under profiles/."""
+    import bench
+    t = bench.traffic_bytes("config4-sweep-2+2", "f64")
+    assert sorted(t) == [0, 1, 2, 3]
+    algorithmic = 2 * 5435817984 * 8
+    for d, b in t.items():
+        assert 0.99 * algorithmic <= b <= 1.02 * algorithmic, (d, b)     # no kernel re-reads f
+    assert bench.traffic_bytes("no-such-workload", "f64") == {}
