@@ -126,6 +126,14 @@ int sldg_advect_pair(sldg_ctx *ctx, int dim1, int dim2, double dt);
 int sldg_translate_pair_dev(sldg_ctx *ctx, int dim1, const double *shift1_device, size_t count1,
                             int dim2, const double *shift2_device, size_t count2);
 
+/* Did a fused v-sweep run outside its regime?  *seen = 1 when, since sldg_create (or the last call with
+ * reset != 0), a fused pair / triple along v-dimensions -- sldg_advect_pair / _triple, the v-group of sldg_step /
+ * sldg_step_n, the raw fused calls -- was launched on shift tables with at least one line shifted by a cell or more
+ * (|E| dt >= h_v), i.e. some of its blocks took the slow global-read fallback (about 2.5x the time of the single
+ * sweeps where most lines are that wide; results unaffected).  A caller who sees 1 should shorten dt or issue
+ * single sweeps.  The mark is left by the table assembly on the device; this call synchronises the stream. */
+int sldg_wide_shift_seen(sldg_ctx *ctx, int *seen, int reset);
+
 /* Three consecutive sweeps (dim1 < dim2 < dim3, all x- or all v-dimensions: the 3+3 D step) in one
  * pass over f; identical, bit for bit, to the three single sweeps.  The fused kernel exists for
  * order <= 2; above that the call runs a fused pair followed by a single sweep (same result). */

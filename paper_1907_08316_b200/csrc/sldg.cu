@@ -95,6 +95,7 @@ struct sldg_ctx {
     double *d_part = nullptr;          // [3 + dv][max_splits][X]: rho, f^2, v_a f, |v|^2 f partials
     double *d_scal = nullptr;          // [8]: mass, l2^2, ee, momentum[dv], |v|^2 moment
     int *d_wide = nullptr;             // [1]: some line of a raw fused v-call is shifted by a cell or more
+    int *d_wide_seen = nullptr;        // [1]: sticky -- a fused v-sweep was launched on tables with such a line (sldg_wide_shift_seen)
     // Poisson
     long K[3] = {1, 1, 1}, Mmax[3] = {0, 0, 0}, KK = 1;
     double2 *d_F[3] = {nullptr, nullptr, nullptr}, *d_G[3] = {nullptr, nullptr, nullptr};
@@ -216,7 +217,7 @@ void free_tables(sldg_ctx *c) {
     for (auto &t : c->xt) { cudaFree(t.sigma); cudaFree(t.m); cudaFree(t.ab); }
     cudaFree(c->d_Wv); cudaFree(c->d_Wx); cudaFree(c->d_va); cudaFree(c->d_v2);
     cudaFree(c->d_rho); cudaFree(c->d_s2); cudaFree(c->d_E); cudaFree(c->d_mom);
-    cudaFree(c->d_part); cudaFree(c->d_scal); cudaFree(c->d_wide);
+    cudaFree(c->d_part); cudaFree(c->d_scal); cudaFree(c->d_wide); cudaFree(c->d_wide_seen);
     for (int a = 0; a < 3; ++a) { cudaFree(c->d_F[a]); cudaFree(c->d_G[a]); }
     for (int i = 0; i < 4; ++i) cudaFree(c->d_t[i]);
     cudaFree(c->d_gh[0]); cudaFree(c->d_gh[1]);
@@ -416,6 +417,8 @@ extern "C" int sldg_create(sldg_ctx **out, int dx, int dv, const int *cells, int
     CREATE_TRY(cudaMemset(c->d_s2, 0, c->X * sizeof(double)));
     CREATE_TRY(dalloc(&c->d_scal, 8));
     CREATE_TRY(dalloc(&c->d_wide, 1));
+    CREATE_TRY(dalloc(&c->d_wide_seen, 1));
+    CREATE_TRY(cudaMemset(c->d_wide_seen, 0, sizeof(int)));
     {
         // enough v-splits that X/VEC * splits threads fill the machine several times over (6 waves of 2048/SM: with
         // 1-2 waves the last, partly filled wave cost up to half the pass -- fp32 config 5 had 1.003 waves, 4.6 TB/s)
@@ -623,12 +626,14 @@ int run_sweep_t(sldg_ctx *c, int dim, long count) {
             sweep_x1_kernel<T, O><<<(unsigned)(ngroups * bpg), block, 0, c->stream>>>(
                 in, out, n, ngroups, cpg, cpb, bpg, c->d_m, (const T *)c->d_ab, count, c->N[c->dx]);
         }
-    } else if (dim == 1 && c->dx >= 2 && sizeof(T) == 8 && c->use_tma && c->tune.plane_single && c->cells[0] <= 256 && n >= 3 &&
+    } else if (dim == 1 && c->dx >= 2 && sizeof(T) == 8 && O <= 5 && c->use_tma && c->tune.plane_single && c->cells[0] <= 256 && n >= 3 &&
                ((size_t)O * c->cells[0] * O * sizeof(T)) % 16 == 0 &&
                4 * (((size_t)O * c->cells[0] * O * sizeof(T) + 127) & ~(size_t)127) <= 96 * 1024 && outer < (1L << 31)) {
         // x_2: one block per (x_1,x_2) plane, the plane kernel of the fused x-pair with the x_1 rule skipped (slabs
         // streamed by the copy engine): config 4 dim 1 6.44 -> 6.6 TB/s against the register-window kernel below; fp64
-        // only (fp32, config 4: 5.9 against 6.4 TB/s for the 128-bit register-window kernel)
+        // only (fp32, config 4: 5.9 against 6.4 TB/s for the 128-bit register-window kernel) and o <= 5 (2+2 D, 3.3e9 DOF,
+        // plane / register-window in TB/s: o = 3 6.62 / 6.16, o = 4 6.51 / 6.21, o = 5 6.43 / 5.40, o = 6 4.19 / 5.54 --
+        // at o = 6 the 2 o^2 = 72 coefficients per thread no longer fit beside the window)
         const int n1 = c->cells[0];
         const size_t slot = ((size_t)O * n1 * O * sizeof(T) + 127) & ~(size_t)127;
         long qd2 = 1;                                        // q of a plane: (first element / qd2) % qm2
@@ -756,14 +761,17 @@ int run_pair_t(sldg_ctx *c, int k1, int k2, long count1, long count2) {
     T *out = (T *)c->buf[c->cur ^ 1];
     int block = 128;
     size_t sh = (size_t)2 * O * O * 2 * O * 2 * sizeof(double);
+    // fused v-sweeps are built for |shift| < 1 cell: a wider line costs bandwidth (per-block fallback); the table
+    // assembly leaves a sticky mark the caller can read (sldg_wide_shift_seen)
+    int *seen = k1 >= c->dx ? c->d_wide_seen : nullptr;
     if (!c->skip_asm1) {
         assemble_ab_kernel<T><<<(unsigned)cdiv(count1, block), block, sh, c->stream>>>(
-            c->d_sigma, count1, O, n1, c->d_coef, c->d_m, (T *)c->d_ab);
+            c->d_sigma, count1, O, n1, c->d_coef, c->d_m, (T *)c->d_ab, seen);
         LAUNCH_CHECK(c);
     }
     if (!c->skip_asm2) {
         assemble_ab_kernel<T><<<(unsigned)cdiv(count2, block), block, sh, c->stream>>>(
-            c->d_sigma2, count2, O, n2, c->d_coef, c->d_m2, (T *)c->d_ab2);
+            c->d_sigma2, count2, O, n2, c->d_coef, c->d_m2, (T *)c->d_ab2, seen);
         LAUNCH_CHECK(c);
     }
     long inner1 = 1, midN = 1, outer2 = 1;
@@ -927,7 +935,7 @@ int run_triple_t(sldg_ctx *c, int k1, int k2, int k3, long cnt1, long cnt2, long
     for (int i = 0; i < 3; ++i)
         if (!skip[i]) {
             assemble_ab_kernel<T><<<(unsigned)cdiv(cnt[i], block), block, sh, c->stream>>>(
-                sg[i], cnt[i], O, nn[i], c->d_coef, mm[i], (T *)ab[i]);
+                sg[i], cnt[i], O, nn[i], c->d_coef, mm[i], (T *)ab[i], k1 >= c->dx ? c->d_wide_seen : nullptr);
             LAUNCH_CHECK(c);
         }
     long inner1 = 1, mid12 = 1, mid23 = 1, outer3 = 1;
@@ -1531,6 +1539,17 @@ int run_poisson(sldg_ctx *c, double *E_copy) {
 int run_poisson_fwd(sldg_ctx *c) { return run_poisson(c, nullptr); }
 
 }  // namespace
+
+extern "C" int sldg_wide_shift_seen(sldg_ctx *c, int *seen, int reset) {
+    if (!c || !seen) return SLDG_ERR_ARG;
+    DeviceGuard guard(c);
+    int h = 0;
+    CUDA_TRY(c, cudaMemcpyAsync(&h, c->d_wide_seen, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    if (reset) CUDA_TRY(c, cudaMemsetAsync(c->d_wide_seen, 0, sizeof(int), c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    *seen = h != 0;
+    return SLDG_OK;
+}
 
 extern "C" int sldg_compute_rho(sldg_ctx *c, double *rho_out) {
     if (!c) return SLDG_ERR_ARG;

@@ -19,7 +19,7 @@ EXPORTS = [
     "sldg_node_coords", "sldg_set_initial", "sldg_get_f", "sldg_current", "sldg_fill_uniform",
     "sldg_translate", "sldg_translate_dev", "sldg_advect", "sldg_advect_pair", "sldg_translate_pair_dev", "sldg_advect_triple", "sldg_translate_triple_dev", "sldg_compute_rho", "sldg_poisson_E",
     "sldg_set_E", "sldg_advect_x_rho", "sldg_advect_x_twice", "sldg_step", "sldg_step_n", "sldg_diagnostics", "sldg_moments", "sldg_invariants", "sldg_launch_count",
-    "sldg_rho_noalloc",
+    "sldg_rho_noalloc", "sldg_wide_shift_seen",
 ]
 
 
@@ -63,6 +63,7 @@ def _load():
     lib.sldg_invariants.argtypes = [vp, dp, dp, dp, dp, dp]
     lib.sldg_launch_count.argtypes = [vp]
     lib.sldg_launch_count.restype = C.c_ulonglong
+    lib.sldg_wide_shift_seen.argtypes = [vp, ip, C.c_int]
     lib.sldg_rho_noalloc.argtypes = [vp, C.c_int, C.c_size_t, C.c_size_t, vp, vp, vp, C.c_char_p, C.c_size_t]
     return lib
 
@@ -284,6 +285,13 @@ class Sldg:
         P = (C.c_double * self.dv)()
         self._chk(_lib.sldg_invariants(self.h, C.byref(m), C.byref(l2), C.byref(ee), P, C.byref(k)), "invariants")
         return m.value, l2.value, ee.value, np.array(list(P)), k.value
+
+    def wide_shift_seen(self, reset=False):
+        """True when a fused v-sweep met a line shifted by a cell or more since create / the last reset
+        (it then ran its slow per-block fallback: shorten dt or issue single sweeps).  Synchronises the stream."""
+        seen = C.c_int(0)
+        self._chk(_lib.sldg_wide_shift_seen(self.h, C.byref(seen), 1 if reset else 0), "wide_shift_seen")
+        return bool(seen.value)
 
     def launch_count(self):
         return int(_lib.sldg_launch_count(self.h))

@@ -525,3 +525,35 @@ def test_two_live_contexts_of_different_size_interleaved(o, dtype):
     a.close(); b.close()
     assert np.all(np.isfinite(got))
     assert np.array_equal(got, want)
+
+
+def test_wide_shift_seen_marks_fused_v_sweeps_outside_their_regime():
+    """sldg_wide_shift_seen: the fused v-sweeps never check |E| dt < h_v (they fall back per block, same bits, slower);
+    the table assembly leaves a sticky mark instead, so the cost is not silent.  x-groups and single sweeps, which
+    take any shift in their stride, never raise it."""
+    import torch
+    cfg = W.Config("wide", 2, 2, (8, 6, 8, 8), 3, (0.0, 0.0, -4.0, -4.0), (4 * np.pi, 4 * np.pi, 4.0, 4.0))
+    hv = 1.0                                              # (4 - -4) / 8
+    rng = np.random.default_rng(9)
+    s = make_solver(cfg, "f64")
+    s.set_initial(rng.uniform(0.0, 1.0, cfg.ndof))
+    assert s.wide_shift_seen() is False
+    wide_v = torch.from_numpy(rng.uniform(-3.5, 3.5, cfg.N[2])).cuda()
+    wide_w = torch.from_numpy(rng.uniform(-3.5, 3.5, cfg.N[3])).cuda()
+    s.translate_pair(0, wide_v, 1, wide_w)                # x-pair: any shift is its home ground
+    s.translate(2, rng.uniform(-3.5, 3.5, cfg.X))         # single v-sweep: likewise
+    s.set_E(0.3 * hv * np.sin(np.arange(2 * cfg.X)).reshape(2, cfg.X))
+    s.advect_pair(2, 3, 1.0)                              # |E| dt < h_v: the regime the fused v-pair is built for
+    s.step(0.05)
+    assert s.wide_shift_seen() is False
+    s.set_E(2.5 * hv * np.sin(np.arange(2 * cfg.X)).reshape(2, cfg.X))
+    s.advect_pair(2, 3, 1.0)                              # some lines move by more than a cell
+    assert s.wide_shift_seen(reset=True) is True
+    assert s.wide_shift_seen() is False                   # the reset took
+    small_x = torch.from_numpy(rng.uniform(-0.4, 0.4, cfg.X)).cuda()
+    wide_x = torch.from_numpy(rng.uniform(-2.5, 2.5, cfg.X)).cuda()
+    s.translate_pair(2, small_x, 3, small_x)
+    assert s.wide_shift_seen() is False
+    s.translate_pair(2, small_x, 3, wide_x)               # raw fused v-call, second table wide
+    assert s.wide_shift_seen() is True
+    s.close()
